@@ -1,0 +1,155 @@
+"""Pins for the oracle's voxel traversal and sample placement (readings C, D of DESIGN.md;
+PAPER.md:174 ray casting over occupied voxels, :164 dense sampling of occupied voxels)."""
+import numpy as np
+import pytest
+
+F = np.float32
+
+
+def _rays(sc, n, seed):
+    """Non-degenerate test rays: origins at voxel centre + (0.137,0.291,0.419)*voxel, random directions."""
+    rng = np.random.default_rng(seed)
+    dims = np.array(sc.dims)
+    bmin = np.array(sc.box_min, np.float64)
+    vs = (np.array(sc.box_max, np.float64) - bmin) / dims
+    out = []
+    for _ in range(n):
+        idx = rng.integers(1, dims - 1)
+        o = bmin + (idx + 0.5 + np.array([0.137, 0.291, 0.419]) * 0.5) * vs
+        d = rng.normal(size=3)
+        d /= np.linalg.norm(d)
+        out.append((o.astype(F), d.astype(F)))
+    return out
+
+
+def _brute_force(sc, o, d):
+    """Per-voxel predicate {i : max(t0, max_a tn_a(i)) < min_a tf_a(i)} over ALL voxels, binary32."""
+    nx, ny, nz = sc.dims
+    bmin = np.array(sc.box_min, F)
+    bmax = np.array(sc.box_max, F)
+    vs = (bmax - bmin) / np.array(sc.dims, F)
+    inv = F(1) / d
+    tn, tf = [], []
+    t0, t1 = F(0), F(np.inf)
+    for a, N in enumerate((nx, ny, nz)):
+        k = np.arange(N + 1, dtype=F)
+        planes = (bmin[a] + k * vs[a]).astype(F)
+        t = ((planes - o[a]) * inv[a]).astype(F)
+        near, far = (t[1:], t[:-1]) if d[a] < 0 else (t[:-1], t[1:])
+        tn.append(near)
+        tf.append(far)
+        t0 = max(t0, (t[N] if d[a] < 0 else t[0]))
+        t1 = min(t1, (t[0] if d[a] < 0 else t[N]))
+    TN = np.maximum(np.maximum(tn[2][:, None, None], tn[1][None, :, None]), tn[0][None, None, :])
+    TN = np.maximum(TN, t0)
+    TF = np.minimum(np.minimum(tf[2][:, None, None], tf[1][None, :, None]), tf[0][None, None, :])
+    hit = np.flatnonzero((TN < TF).reshape(-1))
+    tin = TN.reshape(-1)[hit]
+    order = np.argsort(tin, kind="stable")
+    return hit[order], tin[order], TF.reshape(-1)[hit][order], t0, t1
+
+
+def test_walk_equals_brute_force_predicate(oracle, scene1):
+    s = oracle.scene_from(scene1)
+    for o, d in _rays(scene1, 200, 1):
+        v, ti, to = s.walk(o, d)
+        bv, bti, bto, t0, t1 = _brute_force(scene1, o, d)
+        assert np.array_equal(v, bv)
+        assert np.array_equal(ti.view(np.uint32), bti.view(np.uint32))
+        assert np.array_equal(to.view(np.uint32), bto.view(np.uint32))
+        ok, c0, c1 = s.clip(o, d)
+        assert ok and F(c0) == t0 and F(c1) == t1
+
+
+def test_walk_invariants(oracle, scene1):
+    s = oracle.scene_from(scene1)
+    nx, ny, nz = scene1.dims
+    for o, d in _rays(scene1, 200, 2):
+        v, ti, to = s.walk(o, d)
+        ok, t0, t1 = s.clip(o, d)
+        assert t0 == 0.0                                   # camera inside the box
+        assert ti[0] == t0 and to[-1] == F(t1)
+        assert np.array_equal(ti[1:].view(np.uint32), to[:-1].view(np.uint32))   # segments abut bit-exactly
+        assert np.all(ti < to)
+        assert abs(float(np.sum((to - ti).astype(np.float64))) - (t1 - t0)) < 1e-5
+        ix, iy, iz = v % nx, (v // nx) % ny, v // (nx * ny)
+        steps = np.abs(np.diff(ix)) + np.abs(np.diff(iy)) + np.abs(np.diff(iz))
+        # tie-free rays move one face at a time: voxels visited = 1 + sum |delta index|
+        if np.all(steps == 1):
+            assert len(v) == 1 + abs(int(ix[-1]) - int(ix[0])) + abs(int(iy[-1]) - int(iy[0])) + abs(int(iz[-1]) - int(iz[0]))
+        assert np.all(steps >= 1) and np.all(steps <= 3)
+        # direction of travel is monotone per axis
+        for c, da in ((ix, d[0]), (iy, d[1]), (iz, d[2])):
+            assert np.all(np.diff(c) * np.sign(da) >= 0)
+
+
+def test_walk_axis_aligned_hand_list(oracle, scene1):
+    # ray along +x from the centre of voxel (10, 7, 5): crosses voxels 10..31 of that row;
+    # voxel size 0.25 -> first exit at 0.125, then every 0.25
+    s = oracle.scene_from(scene1)
+    nx, ny, nz = scene1.dims
+    o = np.array([-4 + 10.5 * 0.25, -4 + 7.5 * 0.25, -1.5 + 5.5 * 0.25], F)
+    v, ti, to = s.walk(o, np.array([1, 0, 0], F))
+    assert np.array_equal(v, (5 * ny + 7) * nx + np.arange(10, 32))
+    assert np.allclose(to, 0.125 + 0.25 * np.arange(22), atol=1e-6)
+    v, ti, to = s.walk(o, np.array([0, 0, -1], F))
+    assert np.array_equal(v, (np.arange(5, -1, -1) * ny + 7) * nx + 10)
+    v, ti, to = s.walk(o, np.array([0, -1, 0], F))
+    assert np.array_equal(v, (5 * ny + np.arange(7, -1, -1)) * nx + 10)
+
+
+def test_walk_occupied_length_matches_analytic_slabs(oracle, scene1):
+    # independent check in binary64: sum over occupied voxels of the ray/box overlap (slab method)
+    s = oracle.scene_from(scene1)
+    occ = scene1.occupied_mask()
+    nx, ny, nz = scene1.dims
+    bmin = np.array(scene1.box_min)
+    vs = (np.array(scene1.box_max) - bmin) / np.array(scene1.dims)
+    lin = np.flatnonzero(occ)
+    idx = np.stack([lin % nx, (lin // nx) % ny, lin // (nx * ny)], 1)
+    lo = bmin + idx * vs
+    hi = lo + vs
+    for o, d in _rays(scene1, 100, 3):
+        o64, d64 = o.astype(np.float64), d.astype(np.float64)
+        ta, tb = (lo - o64) / d64, (hi - o64) / d64
+        tn = np.minimum(ta, tb).max(1)
+        tf = np.maximum(ta, tb).min(1)
+        L = np.clip(tf - np.maximum(tn, 0.0), 0, None).sum()
+        v, ti, to = s.walk(o, d, only_occupied=True)
+        assert np.all(occ[v])
+        assert abs(float((to.astype(np.float64) - ti).sum()) - L) < 2e-5
+
+
+def test_degenerate_rays(oracle, scene1):
+    s = oracle.scene_from(scene1)
+    # origin outside, pointing away: no interval
+    ok, _, _ = s.clip(np.array([10, 0, 0], F), np.array([1, 0, 0], F))
+    assert not ok
+    assert len(s.walk(np.array([10, 0, 0], F), np.array([1, 0, 0], F))[0]) == 0
+    # origin outside, pointing in: enters at t0 > 0 and crosses the whole row
+    v, ti, to = s.walk(np.array([-10, 0.1, 0.1], F), np.array([1, 0, 0], F))
+    assert len(v) == 32 and ti[0] == 6.0
+    # axis-parallel ray outside the slab of a parallel axis
+    assert len(s.walk(np.array([0, 5, 0], F), np.array([1, 0, 0], F))[0]) == 0
+
+
+def test_samples_follow_reading_D(oracle, scene1):
+    s = oracle.scene_from(scene1)
+    K = scene1.samples_per_voxel
+    W, H = scene1.W, scene1.H
+    pose = scene1.poses[0]
+    lab = scene1.voxel_subfield
+    for i, j in [(0, 0), (13, 7), (40, 20), (63, 31), (32, 16)]:
+        o, d = oracle.ray(pose, W, H, i, j)
+        v, ti, to = s.walk(o, d, only_occupied=True)
+        t, dl, sid = s.ray_samples(pose, W, H, i, j)
+        assert len(t) == K * len(v)                       # count = K x occupied voxels crossed
+        assert np.array_equal(sid, np.repeat(lab[v], K))  # label of the crossed voxel
+        assert np.all(np.diff(t) > 0)                     # front to back
+        t = t.reshape(-1, K).astype(np.float64)
+        dl = dl.reshape(-1, K).astype(np.float64)
+        mid = 0.5 * (ti.astype(np.float64) + to)
+        assert np.allclose(0.5 * (t[:, 0] + t[:, -1]), mid, atol=1e-6)      # symmetric about the centre
+        assert np.allclose(K * dl[:, 0], to.astype(np.float64) - ti, rtol=1e-6)
+        assert np.allclose(t[:, 0], ti + 0.5 * dl[:, 0], atol=1e-6)
+        assert np.allclose(np.diff(t, axis=1), dl[:, :-1], atol=1e-6)
