@@ -1,0 +1,146 @@
+/* r360 -- B200-native equirectangular renderer for a radiance field made of
+ * thousands of tiny local MLPs (the render hot path of 360Roam, arxiv 2208.02705).
+ *
+ * C ABI of libr360.so.  Citations are line numbers of the paper text
+ * and readings listed in DESIGN.md.
+ *
+ * Problem statement (section 5.0.1): given the occupancy map, the
+ * label of every occupied voxel ("each occupied voxel ... labeled to the
+ * corresponding tiny MLP M_k") and the n tiny MLPs, render a 360-degree colour and
+ * depth image for a camera pose by ray casting over occupied voxels, querying the
+ * MLP that owns each sample, and volume rendering (Eq. 4-5).
+ *
+ * Conventions
+ *  - "host" pointers are ordinary CPU memory, read during the call and never kept.
+ *  - "device" pointers are CUDA device memory of the current device (for example
+ *    torch.empty(..., device="cuda").data_ptr()), owned by the caller, written
+ *    in stream order on the stream set with r360_set_stream (default: stream 0).
+ *  - Every entry point returns a status; no exception or abort crosses the ABI.
+ *    On failure outputs are unspecified and *out handles are NULL.
+ *  - A handle may be used from one host thread at a time.
+ *  - r360_render* synchronises the stream once per ray chunk internally (to size
+ *    the sample buffers from the exact segment count); outputs are complete in
+ *    stream order when it returns, the host need not synchronise to enqueue more.
+ */
+#ifndef R360_H
+#define R360_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct r360_scene r360_scene; /* opaque; owns all device memory of a scene */
+
+typedef enum {
+  R360_OK = 0,
+  R360_ERR_INVALID_ARG = 1, /* NULL pointer, non-positive size, unsupported width, non-finite pose ... */
+  R360_ERR_BAD_LABEL = 2,   /* an occupied voxel whose subfield label is outside [0, n_subfields)   */
+  R360_ERR_NONFINITE = 3,   /* NaN/Inf in the weights                                              */
+  R360_ERR_CUDA = 4,        /* a CUDA call failed; r360_last_cuda_error() names it                 */
+  R360_ERR_OOM = 5,         /* device (or host) allocation failed                                  */
+  R360_ERR_CAPACITY = 6     /* a buffer provided by the caller (debug taps) is too small           */
+} r360_status;
+
+/* Scene description.  Geometry: DESIGN.md readings C (grid planes
+ * P_a(k) = box_min_a + k * (box_max_a - box_min_a)/dims_a, binary32).
+ * Network: readings A1-A4 ("6212 parameters"; Table 4 :434-444). */
+typedef struct {
+  int32_t dims[3];            /* Nx,Ny,Nz >= 1; linear voxel index = (iz*Ny+iy)*Nx+ix             */
+  float box_min[3];           /* metres; box_max > box_min per axis (voxels may be anisotropic)    */
+  float box_max[3];
+  int32_t n_subfields;        /* n in [1, 65534]                                                   */
+  int32_t hidden_width;       /* Wd: 32 or 64                                                      */
+  int32_t n_hidden;           /* Hd in [1,8]: trunk layers before the density/feature layer        */
+  int32_t pe_pos_levels;      /* L of F(p): 10 (63 inputs); [0,16] accepted                        */
+  int32_t pe_dir_levels;      /* L of F(d): 4 (27 inputs); [0,8] accepted                          */
+  int32_t samples_per_voxel;  /* K in [1,128]: stratum midpoints per occupied voxel crossed        */
+  float t_threshold;          /* tau >= 0: stop a ray after the first sample with T < tau          */
+  int32_t density_activation; /* 0 = ReLU (Table 4), 1 = softplus                    */
+  uint8_t occ_threshold;      /* voxel occupied iff occupancy[i] >= occ_threshold (>= 1)           */
+} r360_scene_desc;
+
+/* Parameters per subfield for a description (6212 for Wd=32,Hd=2,L=10/4); 0 if invalid. */
+int64_t r360_params_per_subfield(const r360_scene_desc* desc);
+
+/* Create a scene.  All three arrays are HOST pointers and are copied.
+ *  occupancy      uint8[N]  N = Nx*Ny*Nz, quantised occupancy probability
+ *  voxel_subfield int32[N]  label in [0,n) of every occupied voxel; ignored where empty
+ *  weights        float[n*P] per subfield, each layer W[out][in] row-major then b[out], in
+ *                 the order trunk-1 (Wd x (3+6Lp)), trunk-2..Hd (Wd x Wd), density (1 x Wd),
+ *                 feature (Wd x Wd), colour (Wd x (Wd+3+6Ld), input [feature, F(d)]), rgb (3 x Wd)
+ * Errors: INVALID_ARG (NULL, dims < 1, box_max <= box_min, n out of range, Wd not 32/64, K out of
+ * range, tau < 0 or NaN, occ_threshold 0), BAD_LABEL, NONFINITE, OOM, CUDA. */
+r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupancy,
+                              const int32_t* voxel_subfield, const float* weights, r360_scene** out);
+
+/* Free a scene and all its device memory.  NULL is a no-op. */
+void r360_scene_destroy(r360_scene* scene);
+
+/* Render one W x H equirectangular view (Eq. 2-5; steps a1-a10 of DESIGN.md).
+ *  pose       HOST float[12]: row-major 3x4 [R|o], camera (x right, y down, z forward,
+ *             PAPER.md:84) -> world; o = camera centre.  Must be finite.
+ *  out_rgb    DEVICE float[H*W*3], row-major, black background
+ *  out_depth  DEVICE float[H*W], Eq. 4's sum w_i t_i (radial distance; not opacity-normalised)
+ * Errors: INVALID_ARG (NULL, W < 1, H < 1, non-finite pose), OOM, CUDA. */
+r360_status r360_render(r360_scene* scene, const float pose[12], int32_t W, int32_t H,
+                        float* out_rgb, float* out_depth);
+
+/* Same for B poses (HOST float[B*12]); outputs DEVICE float[B*H*W*3], float[B*H*W]. */
+r360_status r360_render_batch(r360_scene* scene, const float* poses, int32_t B, int32_t W, int32_t H,
+                              float* out_rgb, float* out_depth);
+
+/* End-to-end convenience: like r360_render_batch but the outputs are HOST buffers
+ * (float[B*H*W*3], float[B*H*W]); the call copies device -> host and returns when done. */
+r360_status r360_render_batch_host(r360_scene* scene, const float* poses, int32_t B, int32_t W, int32_t H,
+                                   float* out_rgb_host, float* out_depth_host);
+
+/* 0 = fp32 MLP on the FP32 ALUs (default); 1 = bf16 tensor-core MLP (tcgen05, fp32 accumulate). */
+r360_status r360_set_precision(r360_scene* scene, int32_t mode);
+/* CUDA stream (cudaStream_t / CUstream as void*) all work of this scene is enqueued on. */
+r360_status r360_set_stream(r360_scene* scene, void* cuda_stream);
+/* Upper bound on rays processed per internal chunk (default 4 Mi). */
+r360_status r360_set_chunk_rays(r360_scene* scene, int64_t max_rays);
+
+typedef struct {
+  uint64_t rays;             /* of the last render call                                            */
+  uint64_t segments;         /* occupied voxels crossed, summed over rays                          */
+  uint64_t samples_emitted;  /* K * segments (geometric; bit-exact contract)                       */
+  uint64_t samples_used;     /* samples composited before early-out (floating point; not exact)    */
+  uint64_t mlp_tiles;        /* 128-row tiles the MLP kernel processed                             */
+  uint32_t chunks;           /* ray chunks                                                         */
+  uint32_t kernel_launches;  /* kernels of this library launched by the last render call           */
+  float ms_count;            /* device time per stage of the last render call, CUDA events         */
+  float ms_scan;
+  float ms_emit;
+  float ms_mlp;
+  float ms_composite;
+  float ms_total;
+} r360_stats;
+
+/* Statistics of the last render call; synchronises the scene's stream. */
+r360_status r360_get_stats(r360_scene* scene, r360_stats* out);
+
+/* Debug tap for the parity tests (steps a1-a5): runs the sampler and the binning for
+ * one pose and exports, ray-major (ray = j*W + i):
+ *  counts  DEVICE uint32[W*H]   samples of each ray (K x occupied voxels crossed)
+ *  offsets DEVICE uint32[W*H]   exclusive prefix sum of counts
+ *  t       DEVICE float[cap]    sample distances, front to back per ray
+ *  subfield DEVICE int32[cap]   owning subfield of each sample (read back from the bins)
+ *  total   HOST uint64*         total samples; R360_ERR_CAPACITY if total > cap (t/subfield
+ *                               untouched, counts/offsets/total valid) */
+r360_status r360_debug_samples(r360_scene* scene, const float pose[12], int32_t W, int32_t H,
+                               uint32_t* counts, uint32_t* offsets, float* t, int32_t* subfield,
+                               uint64_t cap, uint64_t* total);
+
+const char* r360_status_string(r360_status s);
+/* Text of the last CUDA error seen by this library on the calling thread ("" if none). */
+const char* r360_last_cuda_error(void);
+/* "r360 <version> sm_100a" */
+const char* r360_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

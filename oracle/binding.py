@@ -72,6 +72,8 @@ class Oracle:
                                           _PF, _PF, _PF, _PF, _PF, _PU, _PU]
         L.r360o_render_rows.restype = C.c_int
         L.r360o_render_rows.argtypes = [C.c_void_p, _PF, _I, _I, _I, _I, _PF, _PF, _PF, _PF, _PF, _PU, _PU]
+        L.r360o_samples_rows.restype = C.c_int64
+        L.r360o_samples_rows.argtypes = [C.c_void_p, _PF, _I, _I, _I, _I, _PU, C.c_int64, _PF, _PI]
         L.r360o_num_threads.restype = C.c_int
 
     # ---- scene-independent taps
@@ -189,6 +191,18 @@ class OracleScene:
         n = self.o.lib.r360o_ray_samples(self.h, _p(pose, _F), W, H, i, j, cap, _p(t, _F), _p(dl, _F), _p(sid, _I))
         assert n <= cap
         return t[:n].copy(), dl[:n].copy(), sid[:n].copy()
+
+    def samples_rows(self, pose, W, H, row0=0, row1=None):
+        """(counts uint32[rows*W], t float32[S], subfield int32[S]) ray-major."""
+        pose = np.ascontiguousarray(pose, np.float32).reshape(12)
+        row1 = H if row1 is None else row1
+        counts = np.empty((row1 - row0) * W, np.uint32)
+        total = self.o.lib.r360o_samples_rows(self.h, _p(pose, _F), W, H, row0, row1, _p(counts, _U), 0, None, None)
+        t = np.empty(max(total, 1), np.float32); sid = np.empty(max(total, 1), np.int32)
+        got = self.o.lib.r360o_samples_rows(self.h, _p(pose, _F), W, H, row0, row1, _p(counts, _U), total,
+                                            _p(t, _F), _p(sid, _I))
+        assert got == total
+        return counts, t[:total], sid[:total]
 
     def subfield_frame(self, k):
         c, ih = np.empty(3, np.float32), np.empty(3, np.float32)

@@ -549,6 +549,44 @@ int r360o_render_rows(const r360o_scene* s, const float pose[12], int32_t W, int
   return 0;
 }
 
+/* Bulk form of r360o_ray_samples for image rows [row0,row1): counts[ray] always; when t/subfield
+ * are given they receive the samples ray-major at the exclusive prefix sum of counts (cap = their
+ * length).  Returns the total number of samples, or -1 if it exceeds cap. */
+int64_t r360o_samples_rows(const r360o_scene* s, const float pose[12], int32_t W, int32_t H,
+                           int32_t row0, int32_t row1, uint32_t* counts, int64_t cap, float* t,
+                           int32_t* subfield) {
+  int64_t n_pix = (int64_t)(row1 - row0) * W;
+  float* tab = (float*)malloc((size_t)(2 * W + 2 * H) * sizeof(float));
+  float *sp = tab, *cp = tab + W, *st = tab + 2 * W, *ct = tab + 2 * W + H;
+  r360o_trig_tables(W, H, sp, cp, st, ct);
+  float o[3] = {pose[3], pose[7], pose[11]};
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t q = 0; q < n_pix; ++q) {
+    float d[3];
+    ray_dir(pose, sp[q % W], cp[q % W], st[row0 + q / W], ct[row0 + q / W], d);
+    counts[q] = (uint32_t)ray_samples(s, o, d, 0, NULL, NULL, NULL);
+  }
+  int64_t total = 0;
+  for (int64_t q = 0; q < n_pix; ++q) total += counts[q];
+  if (t && subfield) {
+    if (total > cap) { free(tab); return -1; }
+    int64_t* off = (int64_t*)malloc((size_t)(n_pix + 1) * sizeof(int64_t));
+    off[0] = 0;
+    for (int64_t q = 0; q < n_pix; ++q) off[q + 1] = off[q] + counts[q];
+    float* dl = (float*)malloc((size_t)(total + 1) * sizeof(float));
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t q = 0; q < n_pix; ++q) {
+      float d[3];
+      ray_dir(pose, sp[q % W], cp[q % W], st[row0 + q / W], ct[row0 + q / W], d);
+      ray_samples(s, o, d, counts[q], t + off[q], dl + off[q], subfield + off[q]);
+    }
+    free(dl);
+    free(off);
+  }
+  free(tab);
+  return total;
+}
+
 int r360o_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -103,6 +103,11 @@ int r360o_render_rows(const r360o_scene* s, const float pose[12], int32_t W, int
                       int32_t row0, int32_t row1,
                       float* rgb, float* depth, float* rgb_full, float* depth_full,
                       float* ambiguity, uint32_t* n_emitted, uint32_t* n_used);
+/* Bulk sample tap for rows [row0,row1): counts[(row1-row0)*W]; optional t/subfield (length cap),
+ * ray-major at the exclusive prefix sum of counts.  Returns total samples, -1 if > cap. */
+int64_t r360o_samples_rows(const r360o_scene* s, const float pose[12], int32_t W, int32_t H,
+                           int32_t row0, int32_t row1, uint32_t* counts, int64_t cap, float* t,
+                           int32_t* subfield);
 int r360o_num_threads(void);
 
 #ifdef __cplusplus

@@ -1,0 +1,12 @@
+"""r360 -- B200-native equirectangular renderer for radiance fields made of thousands of
+tiny MLPs (render hot path of 360Roam, arxiv 2208.02705).
+
+Thin ctypes binding over the C ABI in include/r360.h (libr360.so, hand-written CUDA for
+sm_100a).  Argument marshalling only: every step of the path runs in the CUDA kernels.
+There is no CPU fallback; loading fails loudly if the library is missing.
+"""
+from .binding import (R360Error, Scene, Stats, lib, lib_path, params_per_subfield, scene_from, version,
+                      STATUS)
+
+__all__ = ["R360Error", "Scene", "Stats", "lib", "lib_path", "params_per_subfield", "scene_from", "version",
+           "STATUS"]

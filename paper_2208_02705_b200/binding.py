@@ -1,0 +1,238 @@
+"""ctypes binding of libr360.so: same names as include/r360.h, marshalling only."""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "csrc", "libr360.so")
+
+STATUS = {0: "R360_OK", 1: "R360_ERR_INVALID_ARG", 2: "R360_ERR_BAD_LABEL", 3: "R360_ERR_NONFINITE",
+          4: "R360_ERR_CUDA", 5: "R360_ERR_OOM", 6: "R360_ERR_CAPACITY"}
+
+
+class R360Error(RuntimeError):
+    def __init__(self, status, where, detail=""):
+        self.status = int(status)
+        super().__init__(f"{where}: {STATUS.get(self.status, self.status)} {detail}".strip())
+
+
+class Desc(C.Structure):
+    _fields_ = [("dims", C.c_int32 * 3), ("box_min", C.c_float * 3), ("box_max", C.c_float * 3),
+                ("n_subfields", C.c_int32), ("hidden_width", C.c_int32), ("n_hidden", C.c_int32),
+                ("pe_pos_levels", C.c_int32), ("pe_dir_levels", C.c_int32),
+                ("samples_per_voxel", C.c_int32), ("t_threshold", C.c_float),
+                ("density_activation", C.c_int32), ("occ_threshold", C.c_uint8)]
+
+
+class Stats(C.Structure):
+    _fields_ = [("rays", C.c_uint64), ("segments", C.c_uint64), ("samples_emitted", C.c_uint64),
+                ("samples_used", C.c_uint64), ("mlp_tiles", C.c_uint64), ("chunks", C.c_uint32),
+                ("kernel_launches", C.c_uint32), ("ms_count", C.c_float), ("ms_scan", C.c_float),
+                ("ms_emit", C.c_float), ("ms_mlp", C.c_float), ("ms_composite", C.c_float),
+                ("ms_total", C.c_float)]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_}
+
+
+_LIB = None
+
+
+def lib_path():
+    return _SO
+
+
+def lib():
+    """Load libr360.so (built in-tree by paper_2208_02705_b200.build / __graft_entry__.build)."""
+    global _LIB
+    if _LIB is not None:
+        return _LIB
+    if not os.path.exists(_SO):
+        raise ImportError(f"{_SO} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(_SO)
+    vp, i32, f32p = C.c_void_p, C.c_int32, C.POINTER(C.c_float)
+    L.r360_params_per_subfield.restype = C.c_int64
+    L.r360_params_per_subfield.argtypes = [C.POINTER(Desc)]
+    L.r360_scene_create.restype = C.c_int
+    L.r360_scene_create.argtypes = [C.POINTER(Desc), vp, vp, vp, C.POINTER(vp)]
+    L.r360_scene_destroy.restype = None
+    L.r360_scene_destroy.argtypes = [vp]
+    L.r360_render.restype = C.c_int
+    L.r360_render.argtypes = [vp, f32p, i32, i32, vp, vp]
+    L.r360_render_batch.restype = C.c_int
+    L.r360_render_batch.argtypes = [vp, f32p, i32, i32, i32, vp, vp]
+    L.r360_render_batch_host.restype = C.c_int
+    L.r360_render_batch_host.argtypes = [vp, f32p, i32, i32, i32, vp, vp]
+    L.r360_set_precision.restype = C.c_int
+    L.r360_set_precision.argtypes = [vp, i32]
+    L.r360_set_stream.restype = C.c_int
+    L.r360_set_stream.argtypes = [vp, vp]
+    L.r360_set_chunk_rays.restype = C.c_int
+    L.r360_set_chunk_rays.argtypes = [vp, C.c_int64]
+    L.r360_get_stats.restype = C.c_int
+    L.r360_get_stats.argtypes = [vp, C.POINTER(Stats)]
+    L.r360_debug_samples.restype = C.c_int
+    L.r360_debug_samples.argtypes = [vp, f32p, i32, i32, vp, vp, vp, vp, C.c_uint64, C.POINTER(C.c_uint64)]
+    L.r360_status_string.restype = C.c_char_p
+    L.r360_status_string.argtypes = [C.c_int]
+    L.r360_last_cuda_error.restype = C.c_char_p
+    L.r360_version.restype = C.c_char_p
+    _LIB = L
+    return L
+
+
+def version():
+    return lib().r360_version().decode()
+
+
+def _check(st, where):
+    if st != 0:
+        raise R360Error(st, where, lib().r360_last_cuda_error().decode() if st in (4, 5) else "")
+
+
+def make_desc(dims, box_min, box_max, n_subfields, hidden_width=32, n_hidden=2, pe_pos_levels=10,
+              pe_dir_levels=4, samples_per_voxel=8, t_threshold=1e-3, density_activation=1, occ_threshold=1):
+    d = Desc()
+    d.dims[:] = [int(x) for x in dims]
+    d.box_min[:] = [float(x) for x in box_min]
+    d.box_max[:] = [float(x) for x in box_max]
+    d.n_subfields, d.hidden_width, d.n_hidden = int(n_subfields), int(hidden_width), int(n_hidden)
+    d.pe_pos_levels, d.pe_dir_levels = int(pe_pos_levels), int(pe_dir_levels)
+    d.samples_per_voxel, d.t_threshold = int(samples_per_voxel), float(t_threshold)
+    d.density_activation, d.occ_threshold = int(density_activation), int(occ_threshold)
+    return d
+
+
+def params_per_subfield(**kw):
+    kw.setdefault("dims", (1, 1, 1)); kw.setdefault("box_min", (0, 0, 0)); kw.setdefault("box_max", (1, 1, 1))
+    kw.setdefault("n_subfields", 1)
+    return int(lib().r360_params_per_subfield(C.byref(make_desc(**kw))))
+
+
+def _pose_ptr(poses, B):
+    p = np.ascontiguousarray(poses, dtype=np.float32).reshape(B * 12)
+    return p, p.ctypes.data_as(C.POINTER(C.c_float))
+
+
+class Scene:
+    """r360_scene handle.  Device outputs are torch CUDA tensors (torch = device memory only)."""
+
+    def __init__(self, occupancy, voxel_subfield, weights, **desc_kw):
+        self._h = C.c_void_p()
+        self.desc = make_desc(**desc_kw)
+        occ = np.ascontiguousarray(occupancy, dtype=np.uint8).reshape(-1)
+        lab = np.ascontiguousarray(voxel_subfield, dtype=np.int32).reshape(-1)
+        w = np.ascontiguousarray(weights, dtype=np.float32).reshape(-1)
+        N = int(self.desc.dims[0]) * int(self.desc.dims[1]) * int(self.desc.dims[2])
+        P = int(lib().r360_params_per_subfield(C.byref(self.desc)))
+        if P and (occ.size != N or lab.size != N or w.size != P * int(self.desc.n_subfields)):
+            raise R360Error(1, "r360_scene_create", "array sizes do not match the description")
+        st = lib().r360_scene_create(C.byref(self.desc), occ.ctypes.data, lab.ctypes.data, w.ctypes.data,
+                                     C.byref(self._h))
+        _check(st, "r360_scene_create")
+        self.K = int(self.desc.samples_per_voxel)
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib().r360_scene_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def set_precision(self, mode):
+        _check(lib().r360_set_precision(self._h, {"fp32": 0, "bf16": 1}.get(mode, mode)), "r360_set_precision")
+
+    def set_stream(self, cuda_stream_ptr):
+        _check(lib().r360_set_stream(self._h, C.c_void_p(cuda_stream_ptr)), "r360_set_stream")
+
+    def set_chunk_rays(self, n):
+        _check(lib().r360_set_chunk_rays(self._h, int(n)), "r360_set_chunk_rays")
+
+    def use_current_torch_stream(self):
+        import torch
+        self.set_stream(torch.cuda.current_stream().cuda_stream)
+
+    def render(self, pose, W, H, out_rgb=None, out_depth=None):
+        return self.render_batch(np.asarray(pose, np.float32).reshape(1, 12), W, H, out_rgb, out_depth, _single=True)
+
+    def render_batch(self, poses, W, H, out_rgb=None, out_depth=None, _single=False):
+        import torch
+        poses = np.asarray(poses, np.float32)
+        B = poses.size // 12
+        if out_rgb is None:
+            out_rgb = torch.empty((B, H, W, 3), dtype=torch.float32, device="cuda")
+        if out_depth is None:
+            out_depth = torch.empty((B, H, W), dtype=torch.float32, device="cuda")
+        assert out_rgb.is_cuda and out_depth.is_cuda and out_rgb.is_contiguous() and out_depth.is_contiguous()
+        assert out_rgb.numel() == B * H * W * 3 and out_depth.numel() == B * H * W
+        keep, p = _pose_ptr(poses, B)
+        if _single:
+            st = lib().r360_render(self._h, p, W, H, out_rgb.data_ptr(), out_depth.data_ptr())
+            _check(st, "r360_render")
+            return out_rgb.view(H, W, 3), out_depth.view(H, W)
+        st = lib().r360_render_batch(self._h, p, B, W, H, out_rgb.data_ptr(), out_depth.data_ptr())
+        _check(st, "r360_render_batch")
+        return out_rgb, out_depth
+
+    def render_batch_host(self, poses, W, H, out_rgb=None, out_depth=None):
+        """HOST buffers in and out (numpy, ideally pinned): the end-to-end call."""
+        poses = np.asarray(poses, np.float32)
+        B = poses.size // 12
+        if out_rgb is None:
+            out_rgb = np.empty((B, H, W, 3), np.float32)
+        if out_depth is None:
+            out_depth = np.empty((B, H, W), np.float32)
+        keep, p = _pose_ptr(poses, B)
+        st = lib().r360_render_batch_host(self._h, p, B, W, H, out_rgb.ctypes.data, out_depth.ctypes.data)
+        _check(st, "r360_render_batch_host")
+        return out_rgb, out_depth
+
+    def stats(self):
+        s = Stats()
+        _check(lib().r360_get_stats(self._h, C.byref(s)), "r360_get_stats")
+        return s
+
+    def debug_samples(self, pose, W, H, cap=None):
+        """(counts, offsets, t, subfield) as torch CUDA tensors; steps a1-a5 only."""
+        import torch
+        keep, p = _pose_ptr(pose, 1)
+        counts = torch.empty(W * H, dtype=torch.int32, device="cuda")
+        offsets = torch.empty(W * H, dtype=torch.int32, device="cuda")
+        total = C.c_uint64(0)
+        if cap is None:
+            st = lib().r360_debug_samples(self._h, p, W, H, counts.data_ptr(), offsets.data_ptr(), None, None, 0,
+                                          C.byref(total))
+            if st not in (0, 6):
+                _check(st, "r360_debug_samples")
+            cap = int(total.value)
+        t = torch.empty(max(cap, 1), dtype=torch.float32, device="cuda")
+        sid = torch.empty(max(cap, 1), dtype=torch.int32, device="cuda")
+        st = lib().r360_debug_samples(self._h, p, W, H, counts.data_ptr(), offsets.data_ptr(), t.data_ptr(),
+                                      sid.data_ptr(), cap, C.byref(total))
+        _check(st, "r360_debug_samples")
+        n = int(total.value)
+        return counts, offsets, t[:n], sid[:n]
+
+
+def scene_from(sc, **override):
+    """Scene from a scenegen.Scene (data only)."""
+    kw = dict(dims=sc.dims, box_min=sc.box_min, box_max=sc.box_max, n_subfields=sc.n_subfields,
+              hidden_width=sc.hidden_width, n_hidden=sc.n_hidden, pe_pos_levels=sc.pe_pos_levels,
+              pe_dir_levels=sc.pe_dir_levels, samples_per_voxel=sc.samples_per_voxel, t_threshold=sc.t_threshold,
+              density_activation=sc.density_activation, occ_threshold=sc.occ_threshold)
+    arrays = dict(occupancy=sc.occupancy, voxel_subfield=sc.voxel_subfield, weights=sc.weights)
+    for k, v in override.items():
+        (arrays if k in arrays else kw)[k] = v
+    return Scene(**arrays, **kw)

@@ -1,0 +1,55 @@
+// r360 -- per-ray volume compositing with transmittance early-out (step a10).
+// Eq.4: C = sum w_i c_i, D = sum w_i t_i; Eq.5 (:96-99): w_i = T_i alpha_i with
+// alpha_i = 1 - exp(-sigma_i delta_i); readings E (delta_i = the sample's stratum) and G (running
+// product, stop after the first sample with T < tau, black background, depth not normalised).
+#include "kernels.h"
+
+namespace r360 {
+
+__global__ void __launch_bounds__(256)
+k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __restrict__ out_rgb,
+            float* __restrict__ out_depth) {
+  const unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned used = 0;
+  if (r < f.n_rays) {
+    const unsigned cnt = b.ray_cnt[r];
+    const unsigned off = b.ray_off[r];
+    const int K = g.K;
+    float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f;
+    bool done = false;
+    for (unsigned s = 0; s < cnt && !done; ++s) {
+      const float t_in = b.seg_tin[off + s];
+      const float dt = b.seg_dt[off + s];
+      const float4* o = b.out + (size_t)(off + s) * K;
+      for (int j = 0; j < K; ++j) {
+        const float4 v = __ldcs(o + j);
+        const float t = __fmaf_rn((float)j + 0.5f, dt, t_in);
+        const float alpha = 1.0f - expf(-v.x * dt);
+        const float w = T * alpha;
+        C0 = fmaf(w, v.y, C0);
+        C1 = fmaf(w, v.z, C1);
+        C2 = fmaf(w, v.w, C2);
+        D = fmaf(w, t, D);
+        T = T * (1.0f - alpha);
+        ++used;
+        if (T < tau) { done = true; break; }
+      }
+    }
+    const size_t gr = (size_t)(f.ray0 + (long long)r);
+    out_rgb[gr * 3 + 0] = C0;
+    out_rgb[gr * 3 + 1] = C1;
+    out_rgb[gr * 3 + 2] = C2;
+    out_depth[gr] = D;
+  }
+  // samples_used statistic
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) used += __shfl_xor_sync(0xffffffffu, used, o);
+  if ((threadIdx.x & 31) == 0 && used) atomicAdd(&b.totals[2], (unsigned long long)used);
+}
+
+void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
+                      float* out_rgb, float* out_depth, cudaStream_t s) {
+  k_composite<<<(f.n_rays + 255) / 256, 256, 0, s>>>(g, f, b, tau, out_rgb, out_depth);
+}
+
+}  // namespace r360

@@ -1,0 +1,75 @@
+// r360 -- host-side launch wrappers of the CUDA kernels (one per pipeline stage).
+#pragma once
+#include "common.cuh"
+
+namespace r360 {
+
+// Per-subfield constants in device memory.
+struct SubfieldFrame {      // reading A3: q = (p - centre) * inv_half
+  float cx, cy, cz, pad0;
+  float ix, iy, iz, pad1;
+};
+
+// Network shape shared by the MLP kernels.
+struct NetShape {
+  int Wd;        // hidden width (32 / 64)
+  int Hd;        // trunk layers
+  int Lp, Ld;    // PE levels
+  int pe_p, pe_d;
+  int act;       // 0 ReLU, 1 softplus
+  int P;         // parameters per subfield (fp32 blob, transposed layout has the same size)
+};
+
+// Device layout of one subfield's fp32 weights for the ALU kernel (float offsets; every block
+// is padded to a multiple of 4 floats so rows can be read as float4):
+//   trunk l : W^T[in][Wd] then b[Wd]        density : w[Wd] then b, pad 3
+//   feature : W^T[Wd][Wd] then b[Wd]        colour  : W^T[Wd+pe_d][Wd] then b[Wd]
+//   rgb     : W^T[Wd][4] (r,g,b,0) then b[4]
+struct Fp32Layout {
+  int trunk[8];
+  int dens, feat, col, rgb;
+  int total;
+};
+
+// Device buffers of one ray chunk.
+struct ChunkBuffers {
+  uint32_t* ray_cnt;     // [n_rays] segments per ray
+  uint32_t* ray_off;     // [n_rays] block-local exclusive offset after count; global after emit
+  uint32_t* block_sum;   // [n_blocks] segments per sampler block -> exclusive scan in place
+  uint32_t* bin_cnt;     // [n] segments per subfield
+  uint32_t* bin_start;   // [n+1]
+  uint32_t* bin_cursor;  // [n]
+  uint32_t* tile_start;  // [n+1] first MLP tile of each subfield
+  unsigned long long* totals;  // [4]: segments, tiles, samples_used (accumulated), spare
+  float* seg_tin;        // [G] ray-major
+  float* seg_dt;         // [G] ray-major
+  SegRec* recs;          // [G] binned by subfield
+  float4* out;           // [G*K] (sigma, r, g, b) per sample, ray-major
+};
+
+constexpr int kSamplerThreads = 256;
+
+void launch_count(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
+                  int n_bins, cudaStream_t s);
+void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_tile, cudaStream_t s);
+void launch_emit(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
+                 cudaStream_t s);
+// fp32 MLP on the FP32 ALUs.  weights_t: per subfield, per layer W^T[in][out] then b[out].
+cudaError_t launch_mlp_fp32(const GridParams& g, const FrameParams& f, const ChunkBuffers& b,
+                            const NetShape& net, const Fp32Layout& lay, const float* weights_t,
+                            const SubfieldFrame* frames, int n_bins, int segs_per_tile, int n_sms,
+                            cudaStream_t s);
+// bf16 tensor-core MLP (tcgen05).  wpack: per subfield packed bf16 operand tiles + fp32 biases.
+cudaError_t launch_mlp_tc(const GridParams& g, const FrameParams& f, const ChunkBuffers& b,
+                          const NetShape& net, const void* wpack, size_t wpack_stride,
+                          const SubfieldFrame* frames, int n_bins, int segs_per_tile, int n_sms,
+                          cudaStream_t s);
+void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
+                      float* out_rgb, float* out_depth, cudaStream_t s);
+// debug: expand binned records into ray-major per-sample t and subfield id
+void launch_export_samples(const GridParams& g, const ChunkBuffers& b, int n_bins, unsigned n_segs,
+                           float* t, int32_t* subfield, cudaStream_t s);
+void launch_export_counts(const ChunkBuffers& b, unsigned n_rays, int K, uint32_t* counts, uint32_t* offsets,
+                          cudaStream_t s);
+
+}  // namespace r360

@@ -1,0 +1,248 @@
+// r360 -- ray generation + occupancy DDA sampler, and the binning by subfield (steps a1-a5).
+//
+// Two walks per ray, no intermediate ray-major record stream:
+//   k_count : walk #1  -> segments per ray, block-local exclusive offsets, per-subfield histogram
+//   k_scan  : one launch, two blocks: exclusive scan of the block sums; exclusive scan of the
+//             histogram (bin starts) and of the per-subfield MLP tile counts
+//   k_emit  : walk #2  -> each segment goes straight to its bin (warp-aggregated cursor atomics);
+//             the ray-major (t_in, delta) pair is kept for the compositing kernel
+// A "segment" is one occupied voxel crossed by one ray; it stands for K samples (reading D).
+// PAPER.md:174 (ray casting to localise occupied voxels, per-voxel tiny-MLP label), :164, :29.
+#include "kernels.h"
+
+namespace r360 {
+
+__device__ __forceinline__ unsigned lanemask_lt() {
+  unsigned m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
+
+// Block-wide exclusive scan of one value per thread (blockDim.x = kSamplerThreads).
+__device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* warp_sums, uint32_t& total) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  uint32_t incl = x;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += y;
+  }
+  if (lane == 31) warp_sums[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    uint32_t w = lane < (int)(blockDim.x >> 5) ? warp_sums[lane] : 0;
+    uint32_t wi = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      uint32_t y = __shfl_up_sync(0xffffffffu, wi, o);
+      if (lane >= o) wi += y;
+    }
+    warp_sums[lane] = wi - w;          // exclusive warp offsets
+    if (lane == 31) warp_sums[32] = wi;  // block total
+  }
+  __syncthreads();
+  total = warp_sums[32];
+  return warp_sums[wid] + incl - x;
+}
+
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kSamplerThreads)
+k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuffers b, int n_bins,
+        int use_smem_hist) {
+  extern __shared__ uint32_t hist[];     // [n_bins] when use_smem_hist
+  __shared__ uint32_t warp_sums[33];
+  if (use_smem_hist) {
+    for (int k = threadIdx.x; k < n_bins; k += blockDim.x) hist[k] = 0;
+    __syncthreads();
+  }
+  const unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = r < f.n_rays;
+  Walker w;
+  w.alive = false;
+  if (valid) w.init(g, make_ray(f, r));
+  uint32_t cnt = 0;
+  // lock-step over "next occupied voxel" so the histogram update can be warp-aggregated
+  while (__any_sync(0xffffffffu, w.alive)) {
+    uint32_t lab = 0;
+    float t_in, t_out;
+    bool hit = w.next(g, grid, lab, t_in, t_out);
+    unsigned m = __ballot_sync(0xffffffffu, hit);
+    if (hit) {
+      ++cnt;
+      unsigned peers = __match_any_sync(m, lab);
+      if ((peers & lanemask_lt()) == 0) {
+        uint32_t c = __popc(peers);
+        if (use_smem_hist) atomicAdd(&hist[lab], c);
+        else atomicAdd(&b.bin_cnt[lab], c);
+      }
+    }
+  }
+  uint32_t total;
+  uint32_t off = block_exclusive_scan(cnt, warp_sums, total);
+  if (valid) {
+    b.ray_cnt[r] = cnt;
+    b.ray_off[r] = off;
+  }
+  if (threadIdx.x == 0) b.block_sum[blockIdx.x] = total;
+  if (use_smem_hist) {
+    __syncthreads();
+    for (int k = threadIdx.x; k < n_bins; k += blockDim.x) {
+      uint32_t c = hist[k];
+      if (c) atomicAdd(&b.bin_cnt[k], c);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// Single-block exclusive scan over m values (in -> out, may alias); returns the total to all
+// threads.  blockDim.x = 1024.
+__device__ uint64_t scan_array(const uint32_t* in, uint32_t* out, int m, uint32_t* sm /*[34]*/,
+                               int tile_div /*0: raw values; >0: scan ceil(v/tile_div)*/,
+                               const uint32_t* src_for_tiles) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  uint64_t carry = 0;
+  for (int base = 0; base < m; base += 1024) {
+    int i = base + threadIdx.x;
+    uint32_t x = 0;
+    if (i < m) {
+      x = tile_div ? (src_for_tiles[i] + tile_div - 1) / tile_div : in[i];
+    }
+    uint32_t incl = x;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += y;
+    }
+    if (lane == 31) sm[wid] = incl;
+    __syncthreads();
+    if (wid == 0) {
+      uint32_t w = sm[lane], wi = w;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        uint32_t y = __shfl_up_sync(0xffffffffu, wi, o);
+        if (lane >= o) wi += y;
+      }
+      sm[lane] = wi - w;
+      if (lane == 31) sm[32] = wi;
+    }
+    __syncthreads();
+    if (i < m) out[i] = (uint32_t)(carry + sm[wid] + incl - x);
+    carry += sm[32];
+    __syncthreads();
+  }
+  return carry;
+}
+
+__global__ void __launch_bounds__(1024)
+k_scan(ChunkBuffers b, int n_blocks, int n_bins, int segs_per_tile) {
+  __shared__ uint32_t sm[34];
+  if (blockIdx.x == 0) {
+    uint64_t tot = scan_array(b.block_sum, b.block_sum, n_blocks, sm, 0, nullptr);
+    if (threadIdx.x == 0) b.totals[0] = tot;
+  } else {
+    // tile counts first (they read bin_cnt), then the bin starts
+    uint64_t tiles = scan_array(nullptr, b.tile_start, n_bins, sm, segs_per_tile, b.bin_cnt);
+    uint64_t segs = scan_array(b.bin_cnt, b.bin_start, n_bins, sm, 0, nullptr);
+    if (threadIdx.x == 0) {
+      b.tile_start[n_bins] = (uint32_t)tiles;
+      b.bin_start[n_bins] = (uint32_t)segs;
+      b.totals[1] = tiles;
+    }
+    for (int k = threadIdx.x; k < n_bins; k += blockDim.x) b.bin_cursor[k] = 0;
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kSamplerThreads)
+k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuffers b) {
+  const unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool valid = r < f.n_rays;
+  Walker w;
+  w.alive = false;
+  uint32_t slot = 0;
+  if (valid) {
+    w.init(g, make_ray(f, r));
+    slot = b.block_sum[blockIdx.x] + b.ray_off[r];
+    b.ray_off[r] = slot;                 // now the global ray-major offset
+  }
+  while (__any_sync(0xffffffffu, w.alive)) {
+    uint32_t lab = 0;
+    float t_in = 0.f, t_out = 0.f;
+    bool hit = w.next(g, grid, lab, t_in, t_out);
+    unsigned m = __ballot_sync(0xffffffffu, hit);
+    if (hit) {
+      // reading D: delta = (t_out - t_in) / K, one subtract, one divide
+      float dt = __fdiv_rn(__fsub_rn(t_out, t_in), g.Kf);
+      unsigned peers = __match_any_sync(m, lab);
+      int leader = __ffs(peers) - 1;
+      uint32_t base = 0;
+      if ((int)(threadIdx.x & 31) == leader) base = atomicAdd(&b.bin_cursor[lab], (uint32_t)__popc(peers));
+      base = __shfl_sync(peers, base, leader);
+      uint32_t pos = __ldg(b.bin_start + lab) + base + __popc(peers & lanemask_lt());
+      b.recs[pos] = make_uint4(r, __float_as_uint(t_in), __float_as_uint(dt), slot);
+      b.seg_tin[slot] = t_in;
+      b.seg_dt[slot] = dt;
+      ++slot;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+// debug taps
+__global__ void k_export_samples(GridParams g, ChunkBuffers b, int n_bins, unsigned n_segs, float* t,
+                                 int32_t* subfield) {
+  unsigned pos = blockIdx.x * blockDim.x + threadIdx.x;
+  if (pos >= n_segs) return;
+  // subfield of a bin position: last k with bin_start[k] <= pos
+  int lo = 0, hi = n_bins;
+  while (hi - lo > 1) {
+    int mid = (lo + hi) >> 1;
+    if (b.bin_start[mid] <= pos) lo = mid; else hi = mid;
+  }
+  SegRec rec = b.recs[pos];
+  float t_in = __uint_as_float(rec.y), dt = __uint_as_float(rec.z);
+  size_t s0 = (size_t)rec.w * g.K;
+  for (int j = 0; j < g.K; ++j) {
+    t[s0 + j] = __fmaf_rn((float)j + 0.5f, dt, t_in);
+    subfield[s0 + j] = lo;
+  }
+}
+
+__global__ void k_export_counts(ChunkBuffers b, unsigned n_rays, int K, uint32_t* counts, uint32_t* offsets) {
+  unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
+  if (r >= n_rays) return;
+  counts[r] = b.ray_cnt[r] * K;
+  offsets[r] = b.ray_off[r] * K;
+}
+
+// ---------------------------------------------------------------------------------------
+void launch_count(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
+                  int n_bins, cudaStream_t s) {
+  int blocks = (f.n_rays + kSamplerThreads - 1) / kSamplerThreads;
+  int use_smem = n_bins <= 8192;
+  size_t smem = use_smem ? (size_t)n_bins * sizeof(uint32_t) : 0;
+  k_count<<<blocks, kSamplerThreads, smem, s>>>(g, grid, f, b, n_bins, use_smem);
+}
+
+void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_tile, cudaStream_t s) {
+  k_scan<<<2, 1024, 0, s>>>(b, n_blocks, n_bins, segs_per_tile);
+}
+
+void launch_emit(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
+                 cudaStream_t s) {
+  int blocks = (f.n_rays + kSamplerThreads - 1) / kSamplerThreads;
+  k_emit<<<blocks, kSamplerThreads, 0, s>>>(g, grid, f, b);
+}
+
+void launch_export_samples(const GridParams& g, const ChunkBuffers& b, int n_bins, unsigned n_segs,
+                           float* t, int32_t* subfield, cudaStream_t s) {
+  if (!n_segs) return;
+  k_export_samples<<<(n_segs + 255) / 256, 256, 0, s>>>(g, b, n_bins, n_segs, t, subfield);
+}
+
+void launch_export_counts(const ChunkBuffers& b, unsigned n_rays, int K, uint32_t* counts, uint32_t* offsets,
+                          cudaStream_t s) {
+  k_export_counts<<<(n_rays + 255) / 256, 256, 0, s>>>(b, n_rays, K, counts, offsets);
+}
+
+}  // namespace r360

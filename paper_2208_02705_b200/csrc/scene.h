@@ -1,0 +1,53 @@
+// r360 -- host-side scene object behind the opaque r360_scene handle.
+#pragma once
+#include <vector>
+
+#include "../../include/r360.h"
+#include "kernels.h"
+
+struct r360_scene {
+  r360_scene_desc desc;
+  r360::GridParams grid_p;
+  r360::NetShape net;
+  r360::Fp32Layout lay;
+  int n_sms = 148;
+  int segs_per_tile = 16;
+  // scene-constant device data
+  uint16_t* d_grid = nullptr;               // fused occupancy + label, 0xFFFF = empty
+  r360::SubfieldFrame* d_frames = nullptr;  // [n]
+  float* d_wt = nullptr;                    // [n * lay.total] fp32, transposed + padded
+  void* d_wpack = nullptr;                  // [n * wpack_stride] bf16 operand tiles + fp32 biases
+  size_t wpack_stride = 0;
+  // per (W,H): trig tables; per call: poses
+  float* d_tables = nullptr;
+  int tab_W = 0, tab_H = 0;
+  float* d_poses = nullptr;
+  int poses_cap = 0;
+  // chunk buffers and capacities
+  r360::ChunkBuffers buf{};
+  size_t ray_cnt_cap = 0, ray_off_cap = 0, blocks_cap = 0;
+  size_t seg_tin_cap = 0, seg_dt_cap = 0, recs_cap = 0, out_cap = 0;
+  unsigned long long* h_totals = nullptr;   // pinned [4]
+  // D2H staging for r360_render_batch_host
+  float* d_stage_rgb = nullptr;
+  float* d_stage_depth = nullptr;
+  size_t stage_rays_cap = 0;
+  // configuration
+  cudaStream_t stream = nullptr;
+  int precision = 0;
+  long long chunk_rays = 4ll << 20;
+  // statistics of the last call
+  struct ChunkEvents { cudaEvent_t e[6]; };
+  std::vector<ChunkEvents> events;   // pool, one set per chunk
+  unsigned chunks_last = 0;
+  r360_stats stats{};
+};
+
+// records the CUDA error text for r360_last_cuda_error() and maps it to a status
+r360_status r360_cuda_fail(cudaError_t e, const char* what);
+
+#define R360_CUDA(call)                                         \
+  do {                                                          \
+    cudaError_t e_ = (call);                                    \
+    if (e_ != cudaSuccess) return r360_cuda_fail(e_, #call);    \
+  } while (0)

@@ -1,0 +1,40 @@
+"""Helpers of the -m gpu parity tests: compare the CUDA path (through the C ABI binding) with the oracle."""
+import numpy as np
+
+from scenegen import weight_layout
+
+
+def with_density_bias(sc, bias):
+    """Copy of a scenegen scene's weights with the density bias replaced (data only)."""
+    w = sc.weights.copy().reshape(sc.n_subfields, -1)
+    o = 0
+    for name, fo, fi in weight_layout(sc.hidden_width, sc.n_hidden, sc.pe_pos_levels, sc.pe_dir_levels):
+        if name == "density":
+            w[:, o + fo * fi] = bias
+        o += fo * fi + fo
+    return w.reshape(-1)
+
+
+def check_image(gpu_rgb, gpu_depth, ref, tol, amb_band=1e-3, depth_tol=None):
+    """Element-by-element comparison with the oracle's outputs for the same pixels.
+
+    Unambiguous rays: |gpu - oracle| <= tol.  Threshold-ambiguous rays (oracle's
+    min_i |T_i - tau|/tau < amb_band, reading G4): any stopping point is valid, so the GPU
+    value must lie between the stopped and the continued oracle results (C and D only grow).
+    Returns (max_err_rgb, max_err_depth, n_ambiguous)."""
+    depth_tol = tol if depth_tol is None else depth_tol
+    g_rgb = np.asarray(gpu_rgb, np.float64).reshape(-1, 3)
+    g_d = np.asarray(gpu_depth, np.float64).reshape(-1)
+    amb = ref["ambiguity"] < amb_band
+    e_rgb = np.abs(g_rgb - ref["rgb"])
+    e_d = np.abs(g_d - ref["depth"])
+    ok = ~amb
+    max_rgb = float(e_rgb[ok].max()) if ok.any() else 0.0
+    max_d = float(e_d[ok].max()) if ok.any() else 0.0
+    assert max_rgb <= tol, f"rgb error {max_rgb:.3e} > {tol}"
+    assert max_d <= depth_tol, f"depth error {max_d:.3e} > {depth_tol}"
+    if amb.any():
+        lo, hi = ref["rgb"][amb] - tol, ref["rgb_full"][amb] + tol
+        assert np.all((g_rgb[amb] >= lo) & (g_rgb[amb] <= hi))
+        assert np.all((g_d[amb] >= ref["depth"][amb] - depth_tol) & (g_d[amb] <= ref["depth_full"][amb] + depth_tol))
+    return max_rgb, max_d, int(amb.sum())

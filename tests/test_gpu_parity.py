@@ -1,0 +1,193 @@
+"""-m gpu: the CUDA path (through the C ABI) against the oracle, element by element.
+
+Bars (BASELINE.json north_star): sample counts / subfield ids / t bit-exact; fp32 RGB and depth
+within 1e-4 absolute; bf16 tensor-core RGB within 2e-3 absolute (tests/test_gpu_tc.py)."""
+import numpy as np
+import pytest
+
+from conftest import get_scene
+from gpu_util import check_image, with_density_bias
+
+pytestmark = pytest.mark.gpu
+F = np.float32
+
+
+@pytest.fixture(scope="module")
+def r360():
+    import torch
+    assert torch.cuda.is_available()
+    import __graft_entry__ as g
+    g.build()
+    import paper_2208_02705_b200 as m
+    return m
+
+
+def _cmp_samples(r360, oracle, sc, pose, W, H, **override):
+    gpu = r360.scene_from(sc, **override)
+    kw = {k: v for k, v in override.items()}
+    ora = oracle.scene_from(sc) if not kw else None
+    assert ora is not None
+    counts, offsets, t, sid = gpu.debug_samples(pose, W, H)
+    oc, ot, osid = ora.samples_rows(pose, W, H)
+    counts, offsets = counts.cpu().numpy().view(np.uint32), offsets.cpu().numpy().view(np.uint32)
+    assert np.array_equal(counts, oc)                                           # bit-exact counts
+    assert np.array_equal(offsets.astype(np.int64), np.concatenate([[0], np.cumsum(oc.astype(np.int64))[:-1]]))
+    assert np.array_equal(t.cpu().numpy().view(np.uint32), ot.view(np.uint32))  # bit-exact distances
+    assert np.array_equal(sid.cpu().numpy(), osid)                              # exact subfield ids
+    gpu.close()
+    return int(oc.sum())
+
+
+def test_sampler_bit_exact_config1(r360, oracle, scene1):
+    n = _cmp_samples(r360, oracle, scene1, scene1.poses[0], scene1.W, scene1.H)
+    assert n == 39808
+
+
+def test_sampler_bit_exact_config2(r360, oracle, scene2):
+    _cmp_samples(r360, oracle, scene2, scene2.poses[0], scene2.W, scene2.H)
+
+
+@pytest.mark.parametrize("W,H", [(1, 1), (37, 19), (257, 3), (2, 200)])
+def test_sampler_ragged_sizes(r360, oracle, scene1, W, H):
+    _cmp_samples(r360, oracle, scene1, scene1.poses[0], W, H)
+
+
+def test_sampler_camera_outside_and_rotated(r360, oracle, scene1):
+    # outside the box (t0 > 0 for rays that enter, no samples for rays that miss), tilted pose
+    a, b = 0.3, -0.7
+    ra = np.array([[1, 0, 0], [0, np.cos(a), -np.sin(a)], [0, np.sin(a), np.cos(a)]])
+    rb = np.array([[np.cos(b), 0, np.sin(b)], [0, 1, 0], [-np.sin(b), 0, np.cos(b)]])
+    pose = np.concatenate([ra @ rb, np.array([[7.3], [-1.1], [0.4]])], 1).astype(F).reshape(12)
+    n = _cmp_samples(r360, oracle, scene1, pose, 96, 48)
+    assert n > 0
+
+
+def _render_cmp(r360, oracle, sc, tol=1e-4, precision="fp32", weights=None, W=None, H=None, **desc_over):
+    W = W or sc.W
+    H = H or sc.H
+    over = dict(desc_over)
+    if weights is not None:
+        over["weights"] = weights
+    gpu = r360.scene_from(sc, **over)
+    gpu.set_precision(precision)
+    okw = dict(dims=sc.dims, box_min=sc.box_min, box_max=sc.box_max, n_subfields=sc.n_subfields,
+               hidden_width=sc.hidden_width, n_hidden=sc.n_hidden, pe_pos_levels=sc.pe_pos_levels,
+               pe_dir_levels=sc.pe_dir_levels, samples_per_voxel=sc.samples_per_voxel,
+               t_threshold=sc.t_threshold, density_activation=sc.density_activation,
+               occ_threshold=sc.occ_threshold, occupancy=sc.occupancy, voxel_subfield=sc.voxel_subfield,
+               weights=sc.weights if weights is None else weights)
+    okw.update(desc_over)
+    ora = oracle.scene(**okw)
+    rgb, depth = gpu.render(sc.poses[0], W, H)
+    ref = ora.render_rows(sc.poses[0], W, H)
+    st = gpu.stats()
+    assert st.samples_emitted == int(ref["n_emitted"].sum())
+    assert st.rays == W * H
+    res = check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, tol)
+    gpu.close()
+    return res, st, ref
+
+
+def test_render_fp32_config1(r360, oracle, scene1):
+    (e_rgb, e_d, n_amb), st, ref = _render_cmp(r360, oracle, scene1)
+    assert st.samples_used == st.samples_emitted == 39808
+    assert st.kernel_launches == 5
+
+
+def test_render_fp32_config2(r360, oracle, scene2):
+    _render_cmp(r360, oracle, scene2)
+
+
+def test_render_fp32_early_out(r360, oracle, scene1):
+    # dense medium: most rays stop early; the stopping sample must match the oracle's
+    w = with_density_bias(scene1, 40.0)
+    (e_rgb, e_d, n_amb), st, ref = _render_cmp(r360, oracle, scene1, weights=w)
+    assert st.samples_used < st.samples_emitted
+    amb = ref["ambiguity"] < 1e-3
+    if not amb.any():
+        assert st.samples_used == int(ref["n_used"].sum())
+
+
+@pytest.mark.parametrize("over", [dict(samples_per_voxel=12), dict(samples_per_voxel=5),
+                                  dict(samples_per_voxel=1), dict(samples_per_voxel=128),
+                                  dict(density_activation=0), dict(t_threshold=0.0)])
+def test_render_fp32_variants(r360, oracle, scene1, over):
+    _render_cmp(r360, oracle, scene1, **over)
+
+
+def test_render_fp32_width64_hidden3(r360, oracle):
+    from scenegen import mlp_param_count
+    sc = get_scene(1)
+    P = mlp_param_count(64, 3)
+    rng = np.random.default_rng(7)
+    w = rng.uniform(-0.25, 0.25, sc.n_subfields * P).astype(F)
+    _render_cmp(r360, oracle, sc, weights=w, hidden_width=64, n_hidden=3)
+
+
+def test_empty_scene_is_black(r360, scene1):
+    import torch
+    sc = scene1
+    gpu = r360.scene_from(sc, occupancy=np.zeros_like(sc.occupancy))
+    rgb, depth = gpu.render(sc.poses[0], 64, 32)
+    assert torch.all(rgb == 0) and torch.all(depth == 0)
+    assert gpu.stats().samples_emitted == 0
+
+
+def test_chunked_and_batched_equal_single(r360, scene1):
+    import torch
+    sc = scene1
+    gpu = r360.scene_from(sc)
+    rgb0, d0 = gpu.render(sc.poses[0], 64, 32)
+    rgb0, d0 = rgb0.clone(), d0.clone()
+    gpu.set_chunk_rays(300)                                     # 7 ragged chunks
+    rgb1, d1 = gpu.render(sc.poses[0], 64, 32)
+    assert gpu.stats().chunks == 7
+    assert torch.equal(rgb0, rgb1) and torch.equal(d0, d1)
+    pose2 = sc.poses[0].copy()
+    pose2[3] += 0.4
+    poses = np.stack([sc.poses[0], pose2])
+    rgbb, db = gpu.render_batch(poses, 64, 32)
+    gpu.set_chunk_rays(1 << 22)
+    rgb2, d2 = gpu.render(pose2, 64, 32)
+    assert torch.equal(rgbb[0], rgb0) and torch.equal(rgbb[1], rgb2) and torch.equal(db[1], d2)
+    h_rgb, h_d = gpu.render_batch_host(poses, 64, 32)
+    assert np.array_equal(h_rgb, rgbb.cpu().numpy()) and np.array_equal(h_d, db.cpu().numpy())
+
+
+def test_render_rejects_bad_arguments(r360, scene1):
+    gpu = r360.scene_from(scene1)
+    bad = scene1.poses[0].copy()
+    bad[5] = np.nan
+    with pytest.raises(r360.R360Error) as e:
+        gpu.render(bad, 64, 32)
+    assert e.value.status == 1
+    L = r360.lib()
+    assert L.r360_render(gpu._h, None, 64, 32, None, None) == 1
+
+
+def test_full_size_config3_sampled(r360, oracle):
+    """BASELINE config 3 in the launch configuration bench.py times: 2048x1024, ~1k subfields.
+    The oracle renders a sample of pixels one by one; counts are compared on whole rows."""
+    sc = get_scene(3)
+    gpu = r360.scene_from(sc)
+    ora = oracle.scene_from(sc)
+    rgb, depth = gpu.render(sc.poses[0], sc.W, sc.H)
+    st = gpu.stats()
+    rng = np.random.default_rng(3)
+    px = rng.integers(0, sc.W, 3000).astype(np.int32)
+    py = rng.integers(0, sc.H, 3000).astype(np.int32)
+    ref = ora.render_pixels(sc.poses[0], sc.W, sc.H, px, py)
+    g_rgb = rgb.cpu().numpy()[py, px]
+    g_d = depth.cpu().numpy()[py, px]
+    check_image(g_rgb, g_d, ref, 1e-4)
+    counts, offsets, t, sid = gpu.debug_samples(sc.poses[0], sc.W, sc.H)
+    counts = counts.cpu().numpy().view(np.uint32).reshape(sc.H, sc.W)
+    assert int(counts.sum()) == st.samples_emitted
+    assert np.array_equal(counts[py, px], ref["n_emitted"])
+    for row in (0, 511, 1023):
+        oc, ot, osid = ora.samples_rows(sc.poses[0], sc.W, sc.H, row, row + 1)
+        assert np.array_equal(counts[row], oc)
+        o0 = int(offsets[row * sc.W].item())
+        n = int(oc.sum())
+        assert np.array_equal(t[o0:o0 + n].cpu().numpy().view(np.uint32), ot.view(np.uint32))
+        assert np.array_equal(sid[o0:o0 + n].cpu().numpy(), osid)
