@@ -1,0 +1,118 @@
+"""-m gpu: the bf16 tensor-core MLP path (tcgen05) against the oracle: RGB within 2e-3 absolute,
+max over pixels (BASELINE.json north_star).  Depth is a sum of w_i * t_i with t up to the scene
+diagonal, so its bound scales with the ray length: 2e-3 * t_max."""
+import numpy as np
+import pytest
+
+from conftest import get_scene
+from gpu_util import check_image, with_density_bias
+
+pytestmark = pytest.mark.gpu
+F = np.float32
+TOL = 2e-3
+
+
+@pytest.fixture(scope="module")
+def r360():
+    import torch
+    assert torch.cuda.is_available()
+    import __graft_entry__ as g
+    g.build()
+    import paper_2208_02705_b200 as m
+    return m
+
+
+def _t_max(sc):
+    return float(np.linalg.norm(np.array(sc.box_max) - np.array(sc.box_min)))
+
+
+def _cmp(r360, oracle, sc, weights=None, amb_band=0.2, px=None, py=None, **desc_over):
+    over = dict(desc_over)
+    if weights is not None:
+        over["weights"] = weights
+    gpu = r360.scene_from(sc, **over)
+    gpu.set_precision("bf16")
+    okw = dict(dims=sc.dims, box_min=sc.box_min, box_max=sc.box_max, n_subfields=sc.n_subfields,
+               hidden_width=sc.hidden_width, n_hidden=sc.n_hidden, pe_pos_levels=sc.pe_pos_levels,
+               pe_dir_levels=sc.pe_dir_levels, samples_per_voxel=sc.samples_per_voxel,
+               t_threshold=sc.t_threshold, density_activation=sc.density_activation,
+               occ_threshold=sc.occ_threshold, occupancy=sc.occupancy, voxel_subfield=sc.voxel_subfield,
+               weights=sc.weights if weights is None else weights)
+    okw.update(desc_over)
+    ora = oracle.scene(**okw)
+    rgb, depth = gpu.render(sc.poses[0], sc.W, sc.H)
+    st = gpu.stats()
+    rgb, depth = rgb.cpu().numpy(), depth.cpu().numpy()
+    if px is None:
+        ref = ora.render_rows(sc.poses[0], sc.W, sc.H)
+        assert st.samples_emitted == int(ref["n_emitted"].sum())
+    else:
+        ref = ora.render_pixels(sc.poses[0], sc.W, sc.H, px, py)
+        rgb, depth = rgb[py, px], depth[py, px]
+    res = check_image(rgb, depth, ref, TOL, amb_band=amb_band, depth_tol=TOL * _t_max(sc))
+    gpu.close()
+    return res
+
+
+def test_sass_has_tcgen05_and_tma():
+    import subprocess
+    import paper_2208_02705_b200 as m
+    sass = subprocess.run(["cuobjdump", "-sass", m.lib_path()], capture_output=True, text=True).stdout
+    assert "UTCHMMA" in sass and "LDTM" in sass and "STTM" in sass and "UBLKCP" in sass
+
+
+def test_render_bf16_config1(r360, oracle, scene1):
+    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1)
+    print("config1 bf16 max rgb err", e_rgb, "depth", e_d)
+
+
+def test_render_bf16_config2(r360, oracle, scene2):
+    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene2)
+    print("config2 bf16 max rgb err", e_rgb, "depth", e_d)
+
+
+@pytest.mark.parametrize("over", [dict(samples_per_voxel=12), dict(samples_per_voxel=5),
+                                  dict(density_activation=0), dict(t_threshold=0.0)])
+def test_render_bf16_variants(r360, oracle, scene1, over):
+    _cmp(r360, oracle, scene1, **over)
+
+
+def test_render_bf16_width64(r360, oracle):
+    from scenegen import mlp_param_count, weight_layout
+    sc = get_scene(1)
+    rng = np.random.default_rng(11)
+    parts = []
+    for name, fo, fi in weight_layout(64, 3):
+        a = np.sqrt(6.0 / (fi + fo))
+        parts.append(rng.uniform(-a, a, (sc.n_subfields, fo * fi)))
+        b = rng.uniform(-0.1, 0.1, (sc.n_subfields, fo))
+        if name == "density":
+            b += 1.0
+        parts.append(b)
+    w = np.concatenate(parts, 1).astype(F).reshape(-1)
+    assert w.size == sc.n_subfields * mlp_param_count(64, 3)
+    _cmp(r360, oracle, sc, weights=w, hidden_width=64, n_hidden=3)
+
+
+def test_render_bf16_early_out(r360, oracle, scene1):
+    # dense medium: the stopping sample depends on sigma (bf16-perturbed); rays whose T passes within
+    # 20 % of tau may legitimately stop one sample earlier or later (reading G4, widened for bf16)
+    _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 40.0), amb_band=0.2)
+
+
+def test_bf16_refused_for_other_pe_sizes(r360, scene1):
+    from scenegen import mlp_param_count
+    sc = scene1
+    P = mlp_param_count(32, 2, 6, 4)
+    gpu = r360.scene_from(sc, weights=np.zeros(sc.n_subfields * P, F), pe_pos_levels=6)
+    with pytest.raises(r360.R360Error):
+        gpu.set_precision("bf16")
+
+
+def test_full_size_config3_bf16_sampled(r360, oracle):
+    sc = get_scene(3)
+    rng = np.random.default_rng(5)
+    px = rng.integers(0, sc.W, 3000).astype(np.int32)
+    py = rng.integers(0, sc.H, 3000).astype(np.int32)
+    e_rgb, e_d, n_amb = _cmp(r360, oracle, sc, px=px, py=py)
+    print("config3 bf16 sampled max rgb err", e_rgb, "depth", e_d)
