@@ -24,6 +24,8 @@ struct GridParams {
 struct FrameParams {
   int W, H;
   long long ray0;        // first global ray of this chunk
+  unsigned pose0;        // ray0 / (W*H)
+  unsigned pix0;         // ray0 % (W*H)
   unsigned n_rays;       // rays in this chunk
   const float* poses;    // device [B*12]
   const float* sin_phi;  // device [W]  (reading B2: host binary64 libm, rounded once)
@@ -44,12 +46,14 @@ struct Ray {
 };
 
 __device__ __forceinline__ Ray make_ray(const FrameParams& f, unsigned r) {
-  long long g = f.ray0 + (long long)r;
-  long long wh = (long long)f.W * f.H;
-  int b = (int)(g / wh);
-  int pix = (int)(g - (long long)b * wh);
-  int j = pix / f.W;
-  int i = pix - j * f.W;
+  // 32-bit index math: a chunk never spans more than 2^31 rays and W*H < 2^31
+  const unsigned wh = (unsigned)f.W * (unsigned)f.H;
+  unsigned pix = f.pix0 + r;
+  unsigned b = pix / wh;
+  pix -= b * wh;
+  b += f.pose0;
+  const unsigned j = pix / (unsigned)f.W;
+  const unsigned i = pix - j * (unsigned)f.W;
   const float* P = f.poses + b * 12;
   float sp = __ldg(f.sin_phi + i), cp = __ldg(f.cos_phi + i);
   float st = __ldg(f.sin_theta + j), ct = __ldg(f.cos_theta + j);

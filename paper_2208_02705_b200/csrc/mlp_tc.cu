@@ -141,7 +141,24 @@ void tc_pack_subfield(const NetShape& net, const float* src_blob, void* dst) {
 // ---------------------------------------------------------------------------------------------
 using namespace tc;
 
-// F(x) for L levels from one accurate sincos per component and the double-angle recurrence
+// sin and cos on |x| <= 1 (normalised positions, reading A3, and unit direction components) by
+// their Taylor polynomials (remainders x^13/13! and x^14/14! are below binary32 resolution).
+__device__ __forceinline__ void sincos_unit(float x, float& s, float& c) {
+  const float x2 = x * x;
+  float ps = fmaf(x2, -2.5052108e-8f, 2.7557319e-6f);     // -1/11!, 1/9!
+  ps = fmaf(x2, ps, -1.9841270e-4f);                      // -1/7!
+  ps = fmaf(x2, ps, 8.3333333e-3f);                       // 1/5!
+  ps = fmaf(x2, ps, -1.6666667e-1f);                      // -1/3!
+  s = fmaf(x * x2, ps, x);
+  float pc = fmaf(x2, 2.0876757e-9f, -2.7557319e-7f);     // 1/12!, -1/10!
+  pc = fmaf(x2, pc, 2.4801587e-5f);                       // 1/8!
+  pc = fmaf(x2, pc, -1.3888889e-3f);                      // -1/6!
+  pc = fmaf(x2, pc, 4.1666667e-2f);                       // 1/4!
+  pc = fmaf(x2, pc, -0.5f);
+  c = fmaf(x2, pc, 1.0f);
+}
+
+// F(x) for L levels from one sincos per component and the double-angle recurrence
 // (s' = 2 s c, c' = 1 - 2 s^2); out[3 + 6l + a] = sin, out[3 + 6l + 3 + a] = cos (reading A2).
 template <int L>
 __device__ __forceinline__ void pe_recurrence(const float x[3], float* out) {
@@ -149,7 +166,7 @@ __device__ __forceinline__ void pe_recurrence(const float x[3], float* out) {
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     out[a] = x[a];
-    sincosf(x[a], &s[a], &c[a]);
+    sincos_unit(x[a], s[a], c[a]);
   }
 #pragma unroll
   for (int l = 0; l < L; ++l) {
@@ -163,6 +180,16 @@ __device__ __forceinline__ void pe_recurrence(const float x[3], float* out) {
       s[a] = s2;
     }
   }
+}
+
+// heads of the bf16 path: ex2/lg2/rcp approximations (relative error ~2^-22, far below bf16)
+__device__ __forceinline__ float fast_sigmoid(float x) {
+  float r;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + __expf(-x)));
+  return r;
+}
+__device__ __forceinline__ float fast_softplus(float x) {
+  return x > 20.0f ? x : __logf(1.0f + __expf(x));
 }
 
 template <int WD>
@@ -242,14 +269,24 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     for (int c = 0; c < WD / 2; c += 16) tmem_st_x16(tA + c, a + c);
   };
 
+  unsigned k_tile_end = 0, k_tile_begin = 0, k_seg_begin = 0, k_seg_end = 0;
+  SubfieldFrame fr = frames[0];
   for (unsigned tile = tile0; tile < tile1; ++tile) {
-    int lo = 0, hi = n_bins;
-    while (hi - lo > 1) {
-      int mid = (lo + hi) >> 1;
-      if (__ldg(b.tile_start + mid) <= tile) lo = mid; else hi = mid;
-    }
-    const int k = lo;
-    if (k != cur_k) {                                        // stage the subfield's weights (TMA bulk copy)
+    if (tile >= k_tile_end || cur_k < 0) {
+      // subfield of this tile: last k with tile_start[k] <= tile (tiles of a CTA are contiguous, so
+      // this search runs once per subfield, not once per tile)
+      int lo = 0, hi = n_bins;
+      while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (__ldg(b.tile_start + mid) <= tile) lo = mid; else hi = mid;
+      }
+      const int k = lo;
+      k_tile_begin = __ldg(b.tile_start + k);
+      k_tile_end = __ldg(b.tile_start + k + 1);
+      k_seg_begin = __ldg(b.bin_start + k);
+      k_seg_end = __ldg(b.bin_start + k + 1);
+      fr = frames[k];
+      // stage the subfield's weights (TMA bulk copy)
       __syncthreads();                                       // every MMA reading the old weights has completed
       if (tid == 0) {
         mbar_expect_tx(&bar_w, (uint32_t)lay.total);
@@ -259,8 +296,8 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
       mbar_wait(&bar_w, par_w);
       par_w ^= 1;
     }
-    const unsigned seg0 = __ldg(b.bin_start + k) + (tile - __ldg(b.tile_start + k)) * spt;
-    const unsigned nseg = min((unsigned)spt, __ldg(b.bin_start + k + 1) - seg0);
+    const unsigned seg0 = k_seg_begin + (tile - k_tile_begin) * spt;
+    const unsigned nseg = min((unsigned)spt, k_seg_end - seg0);
     const int sidx = tid / K, j = tid - sidx * K;
     const bool active = (unsigned)sidx < nseg;
     SegRec rec = make_uint4(0, 0, 0, 0);
@@ -268,7 +305,6 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     const float t_in = __uint_as_float(rec.y), dt = __uint_as_float(rec.z);
     const float t = __fmaf_rn((float)j + 0.5f, dt, t_in);
     const Ray ray = make_ray(f, active ? rec.x : 0u);
-    const SubfieldFrame fr = frames[k];
     float q[3];
     q[0] = __fmul_rn(__fsub_rn(__fmaf_rn(t, ray.d[0], ray.o[0]), fr.cx), fr.ix);
     q[1] = __fmul_rn(__fsub_rn(__fmaf_rn(t, ray.d[1], ray.o[1]), fr.cy), fr.iy);
@@ -326,13 +362,11 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     wait_ld();
     // ---- heads (A4), fp32
     const float sigma_raw = __uint_as_float(sraw[0]);
-    float sigma = net.act == 1 ? (sigma_raw > 20.0f ? sigma_raw : log1pf(expf(sigma_raw)))
-                               : fmaxf(sigma_raw, 0.0f);
     float4 o4;
-    o4.x = sigma;
-    o4.y = 1.0f / (1.0f + expf(-__uint_as_float(craw[0])));
-    o4.z = 1.0f / (1.0f + expf(-__uint_as_float(craw[1])));
-    o4.w = 1.0f / (1.0f + expf(-__uint_as_float(craw[2])));
+    o4.x = net.act == 1 ? fast_softplus(sigma_raw) : fmaxf(sigma_raw, 0.0f);
+    o4.y = fast_sigmoid(__uint_as_float(craw[0]));
+    o4.z = fast_sigmoid(__uint_as_float(craw[1]));
+    o4.w = fast_sigmoid(__uint_as_float(craw[2]));
     if (active) b.out[(size_t)rec.w * K + j] = o4;
   }
   fence_before_sync();

@@ -61,6 +61,8 @@ r360_status upload_poses(r360_scene* sc, const float* poses, int B) {
 FrameParams frame_params(const r360_scene* sc, int W, int H, long long ray0, unsigned n_rays) {
   FrameParams f;
   f.W = W; f.H = H; f.ray0 = ray0; f.n_rays = n_rays;
+  f.pose0 = (unsigned)(ray0 / ((long long)W * H));
+  f.pix0 = (unsigned)(ray0 % ((long long)W * H));
   f.poses = sc->d_poses;
   f.sin_phi = sc->d_tables;
   f.cos_phi = sc->d_tables + W;
@@ -119,6 +121,7 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
 static r360_status render_device(r360_scene* sc, const float* poses, int B, int W, int H, float* out_rgb,
                                  float* out_depth) {
   if (!sc || !poses || !out_rgb || !out_depth || B < 1 || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
+  if ((long long)W * H >= (1ll << 30)) return R360_ERR_INVALID_ARG;
   const long long total_rays = (long long)B * W * H;
   r360_status st;
   if ((st = ensure_tables(sc, W, H)) != R360_OK) return st;
@@ -130,7 +133,7 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
   stats.rays = (uint64_t)total_rays;
   unsigned launches = 0, chunk_idx = 0;
   long long chunk = sc->chunk_rays < 1 ? 1 : sc->chunk_rays;
-  if (chunk > (1ll << 31)) chunk = 1ll << 31;
+  if (chunk > (1ll << 30)) chunk = 1ll << 30;
   for (long long ray0 = 0; ray0 < total_rays; ray0 += chunk, ++chunk_idx) {
     unsigned n_rays = (unsigned)((total_rays - ray0 < chunk) ? (total_rays - ray0) : chunk);
     FrameParams f = frame_params(sc, W, H, ray0, n_rays);
@@ -241,7 +244,7 @@ r360_status r360_get_stats(r360_scene* sc, r360_stats* out) {
 r360_status r360_debug_samples(r360_scene* sc, const float pose[12], int32_t W, int32_t H, uint32_t* counts,
                                uint32_t* offsets, float* t, int32_t* subfield, uint64_t cap, uint64_t* total) {
   if (!sc || !pose || !counts || !offsets || !total || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
-  if ((long long)W * H > (1ll << 31)) return R360_ERR_INVALID_ARG;
+  if ((long long)W * H >= (1ll << 30)) return R360_ERR_INVALID_ARG;
   r360_status st;
   if ((st = ensure_tables(sc, W, H)) != R360_OK) return st;
   if ((st = upload_poses(sc, pose, 1)) != R360_OK) return st;
