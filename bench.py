@@ -186,12 +186,8 @@ def main():
     scene.set_precision(precision)
     scene.use_current_torch_stream()
     # each rank renders its own pose: rank r yaws pose 0 by r * 2pi/world about the world up axis
-    pose = sc.poses[0].copy().reshape(3, 4)
-    if world > 1:
-        a = 2 * np.pi * rank / world
-        rz = np.array([[np.cos(a), -np.sin(a), 0], [np.sin(a), np.cos(a), 0], [0, 0, 1]])
-        pose[:, :3] = (rz @ pose[:, :3].astype(np.float64)).astype(np.float32)
-    pose = pose.reshape(12)
+    from paper_2208_02705_b200.shard import rank_pose
+    pose = rank_pose(sc.poses[0], rank, world)
     W, H = sc.W, sc.H
     rgb = torch.empty((1, H, W, 3), dtype=torch.float32, device="cuda")
     depth = torch.empty((1, H, W), dtype=torch.float32, device="cuda")
