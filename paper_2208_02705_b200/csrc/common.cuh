@@ -43,6 +43,7 @@ typedef uint4 SegRec;
 // rounded (the __f*_rn intrinsics are never contracted into FMAs).
 struct Ray {
   float o[3], d[3];
+  unsigned pose;         // index into FrameParams::poses
 };
 
 __device__ __forceinline__ Ray make_ray(const FrameParams& f, unsigned r) {
@@ -61,6 +62,7 @@ __device__ __forceinline__ Ray make_ray(const FrameParams& f, unsigned r) {
   float y = -st;
   float z = __fmul_rn(ct, cp);
   Ray ray;
+  ray.pose = b;
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     float m0 = __fmul_rn(__ldg(P + a * 4 + 0), x);

@@ -1,6 +1,7 @@
 // r360 -- host-side launch wrappers of the CUDA kernels (one per pipeline stage).
 #pragma once
 #include "common.cuh"
+#include "pe.cuh"
 
 namespace r360 {
 
@@ -45,6 +46,9 @@ struct ChunkBuffers {
   float* seg_dt;         // [G] ray-major
   SegRec* recs;          // [G] binned by subfield
   float4* out;           // [G*K] (sigma, r, g, b) per sample, ray-major
+  // tensor path only (null otherwise):
+  uint4* dirblk;         // [n_rays*4] per ray: [1, 1, F(d), 0..] as 32 bf16 (pe.cuh)
+  uint4* rec_dir;        // [G] binned like recs: (d.x, d.y, d.z, pose index)
 };
 
 constexpr int kSamplerThreads = 256;

@@ -90,6 +90,12 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
   if ((st = grow(sc->buf.ray_cnt, sc->ray_cnt_cap, f.n_rays, 1, 1)) != R360_OK) return st;
   if ((st = grow(sc->buf.ray_off, sc->ray_off_cap, f.n_rays, 1, 1)) != R360_OK) return st;
   if ((st = grow(sc->buf.block_sum, sc->blocks_cap, n_blocks, 1, 1)) != R360_OK) return st;
+  if (sc->precision == 1) {            // tensor path: per-ray records (direction + packed F(d))
+    if ((st = grow(sc->d_dirblk, sc->dirblk_cap, (size_t)f.n_rays * 4, 1, 1)) != R360_OK) return st;
+    sc->buf.dirblk = sc->d_dirblk;
+  } else {
+    sc->buf.dirblk = nullptr;
+  }
   cudaStream_t s = sc->stream;
   R360_CUDA(cudaMemsetAsync(sc->buf.bin_cnt, 0, (size_t)n * 4, s));
   if (ev) cudaEventRecord(ev->e[0], s);
@@ -108,6 +114,11 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
     if ((st = grow(sc->buf.seg_tin, sc->seg_tin_cap, n_segs)) != R360_OK) return st;
     if ((st = grow(sc->buf.seg_dt, sc->seg_dt_cap, n_segs)) != R360_OK) return st;
     if ((st = grow(sc->buf.recs, sc->recs_cap, n_segs)) != R360_OK) return st;
+    sc->buf.rec_dir = nullptr;
+    if (sc->precision == 1) {
+      if ((st = grow(sc->d_rec_dir, sc->rec_dir_cap, n_segs)) != R360_OK) return st;
+      sc->buf.rec_dir = sc->d_rec_dir;
+    }
     launch_emit(sc->grid_p, sc->d_grid, f, sc->buf, s);
     launches += 1;
     R360_CUDA(cudaGetLastError());

@@ -59,7 +59,11 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
   const bool valid = r < f.n_rays;
   Walker w;
   w.alive = false;
-  if (valid) w.init(g, make_ray(f, r));
+  if (valid) {
+    const Ray ray = make_ray(f, r);
+    w.init(g, ray);
+    if (b.dirblk) store_dir_block(b.dirblk + (size_t)r * 4, ray.d);   // tensor path: F(d) once per ray
+  }
   uint32_t cnt = 0;
   // lock-step over "next occupied voxel" so the histogram update can be warp-aggregated
   while (__any_sync(0xffffffffu, w.alive)) {
@@ -160,8 +164,11 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
   Walker w;
   w.alive = false;
   uint32_t slot = 0;
+  uint4 dir = make_uint4(0, 0, 0, 0);
   if (valid) {
-    w.init(g, make_ray(f, r));
+    const Ray ray = make_ray(f, r);
+    w.init(g, ray);
+    dir = make_uint4(__float_as_uint(ray.d[0]), __float_as_uint(ray.d[1]), __float_as_uint(ray.d[2]), ray.pose);
     slot = b.block_sum[blockIdx.x] + b.ray_off[r];
     b.ray_off[r] = slot;                 // now the global ray-major offset
   }
@@ -180,6 +187,7 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
       base = __shfl_sync(peers, base, leader);
       uint32_t pos = __ldg(b.bin_start + lab) + base + __popc(peers & lanemask_lt());
       b.recs[pos] = make_uint4(r, __float_as_uint(t_in), __float_as_uint(dt), slot);
+      if (b.rec_dir) b.rec_dir[pos] = dir;
       b.seg_tin[slot] = t_in;
       b.seg_dt[slot] = dt;
       ++slot;

@@ -4,6 +4,8 @@
 #include <cuda_bf16.h>
 #include <stdint.h>
 
+#include "pe.cuh"
+
 namespace r360 {
 namespace tc {
 
@@ -39,6 +41,11 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) {
   }
+}
+
+// ---- named barrier over one 128-thread tile group (id 1..15; id 0 is __syncthreads) -----------
+__device__ __forceinline__ void group_sync_r(uint32_t id) {
+  asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory");
 }
 
 // ---- TMA 1-D bulk copy global -> shared, completes on an mbarrier (async proxy) ----------
@@ -157,20 +164,6 @@ __device__ __forceinline__ void tmem_st_x16(uint32_t taddr, const uint32_t* r) {
       "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]), "r"(r[9]),
       "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
       : "memory");
-}
-
-// ---- packing -------------------------------------------------------------------------------
-// two fp32 -> packed bf16x2 (lo = first argument = lower K index), round to nearest even
-__device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
-  uint32_t r;
-  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
-  return r;
-}
-// same with ReLU fused into the conversion
-__device__ __forceinline__ uint32_t pack_bf16_relu(float lo, float hi) {
-  uint32_t r;
-  asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
-  return r;
 }
 
 }  // namespace tc
