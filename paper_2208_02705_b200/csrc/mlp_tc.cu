@@ -22,6 +22,7 @@
 // groups synchronise with named barriers only, so the st -> mma -> ld chains of all groups overlap.
 // Heads: reading A4 (Table 4 :438-442), biases of the two head rows added in fp32.
 #include <cstring>
+#include <type_traits>
 #include <vector>
 
 #include "kernels.h"
@@ -267,7 +268,9 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   const float jf = (float)j + 0.5f;
 
   // MMAs of one operand pair: ks K steps, A from TMEM columns a_col.., B blocks of N rows at b_off
-  auto mma_steps = [&](uint32_t d_col, uint32_t a_col, int b_off, int N, uint32_t idesc, int ks) {
+  auto mma_steps = [&](uint32_t d_col, uint32_t a_col, int b_off, int N, uint32_t idesc, auto ks_c) {
+    constexpr int ks = decltype(ks_c)::value;
+#pragma unroll
     for (int s = 0; s < ks; ++s)
       mma_ts(d_col, a_col + 8 * s, smem_desc(sw_addr + b_off + s * S::blk(N), 128, 256), idesc, s > 0);
   };
@@ -345,10 +348,13 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     // ---- trunk-1: A = [F(q), 1]
     store_pe_row(tA, q);
     publish();
-    if (tid == 0) {
-      fence_after_sync();
-      mma_steps(mD, mA, lay.trunk[0], WD, idesc_w, S::KP1 / 16);
-      mma_commit(bar_d);
+    if (warp == 0) {
+      if (elect_one()) {
+        fence_after_sync();
+        mma_steps(mD, mA, lay.trunk[0], WD, idesc_w, std::integral_constant<int, S::KP1 / 16>{});
+        mma_commit(bar_d);
+      }
+      __syncwarp();
     }
     // while the tensor core works: fetch the ray's direction block [1, 1, F(d), 0 0 0]
     uint32_t ad[16];
@@ -366,31 +372,40 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     for (int l = 1; l < net.Hd; ++l) {
       d_to_a(tA + S::A_H);
       publish();
-      if (tid == 0) {
-        fence_after_sync();
-        mma_steps(mD, mA, lay.trunk[l], WD, idesc_w, S::KH / 16);
-        mma_commit(bar_d);
+      if (warp == 0) {
+        if (elect_one()) {
+          fence_after_sync();
+          mma_steps(mD, mA, lay.trunk[l], WD, idesc_w, std::integral_constant<int, S::KH / 16>{});
+          mma_commit(bar_d);
+        }
+        __syncwarp();
       }
       wait_acc();
     }
     // ---- colour (feature layer folded in): A = [h, 1, 1, F(d), 0 0 0]
     d_to_a(tA + S::A_H);
     publish();
-    if (tid == 0) {
-      fence_after_sync();
-      mma_steps(mD, mA, lay.col, WD, idesc_w, S::KC / 16);
-      mma_commit(bar_d);
+    if (warp == 0) {
+      if (elect_one()) {
+        fence_after_sync();
+        mma_steps(mD, mA, lay.col, WD, idesc_w, std::integral_constant<int, S::KC / 16>{});
+        mma_commit(bar_d);
+      }
+      __syncwarp();
     }
     wait_acc();
     // ---- heads: rgb from the colour activation (takes the direction block's columns), density
     //      from h (still in place); both N = 16, accumulators side by side
     d_to_a(tA + S::A_FD);
     publish();
-    if (tid == 0) {
-      fence_after_sync();
-      mma_steps(mD, mA + S::A_FD, lay.rgb, S::NHEAD, idesc_h, WD / 16);
-      mma_steps(mD + S::NHEAD, mA + S::A_H, lay.dens, S::NHEAD, idesc_h, WD / 16);
-      mma_commit(bar_d);
+    if (warp == 0) {
+      if (elect_one()) {
+        fence_after_sync();
+        mma_steps(mD, mA + S::A_FD, lay.rgb, S::NHEAD, idesc_h, std::integral_constant<int, WD / 16>{});
+        mma_steps(mD + S::NHEAD, mA + S::A_H, lay.dens, S::NHEAD, idesc_h, std::integral_constant<int, WD / 16>{});
+        mma_commit(bar_d);
+      }
+      __syncwarp();
     }
     const float4 hb = *reinterpret_cast<const float4*>(sw + lay.head_bias);
     wait_acc();

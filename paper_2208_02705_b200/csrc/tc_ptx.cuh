@@ -48,6 +48,15 @@ __device__ __forceinline__ void group_sync_r(uint32_t id) {
   asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory");
 }
 
+// One lane of a converged warp.  tcgen05.mma must be issued from warp-uniform control flow: under a
+// thread-divergent branch (if (tid == 0)) ptxas wraps every UTCHMMA in an ELECT/BRA.U.ANY loop and the
+// issue costs ~60-130 cycles per instruction instead of ~16 (measured, B200).
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+
 // ---- TMA 1-D bulk copy global -> shared, completes on an mbarrier (async proxy) ----------
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
