@@ -50,7 +50,7 @@ typedef struct {
   int32_t dims[3];            /* Nx,Ny,Nz >= 1; linear voxel index = (iz*Ny+iy)*Nx+ix             */
   float box_min[3];           /* metres; box_max > box_min per axis (voxels may be anisotropic)    */
   float box_max[3];
-  int32_t n_subfields;        /* n in [1, 65534]                                                   */
+  int32_t n_subfields;        /* n in [1, 65280]                                                   */
   int32_t hidden_width;       /* Wd: 32 or 64                                                      */
   int32_t n_hidden;           /* Hd in [1,8]: trunk layers before the density/feature layer        */
   int32_t pe_pos_levels;      /* L of F(p): 10 (63 inputs); [0,16] accepted                        */

@@ -25,7 +25,7 @@ bool desc_ok(const r360_scene_desc* d) {
     if (!(d->box_max[a] > d->box_min[a])) return false;
   }
   if ((long long)d->dims[0] * d->dims[1] * d->dims[2] > (1ll << 31) - 1) return false;
-  if (d->n_subfields < 1 || d->n_subfields > 65534) return false;
+  if (d->n_subfields < 1 || d->n_subfields > kMaxSubfields) return false;
   if (d->hidden_width != 32 && d->hidden_width != 64) return false;
   if (d->n_hidden < 1 || d->n_hidden > 8) return false;
   if (d->pe_pos_levels < 0 || d->pe_pos_levels > 16) return false;
@@ -83,6 +83,46 @@ namespace r360 {
 size_t tc_pack_stride(const NetShape& net);
 void tc_pack_subfield(const NetShape& net, const float* src_blob, void* dst);
 }  // namespace r360
+
+// Skip distances of the empty voxels (common.cuh: grid encoding): D = min(255, chessboard distance to
+// the nearest occupied voxel), by the two-pass 26-neighbour chamfer transform, which is exact for the
+// chessboard metric.  Occupied voxels (value < kEmptyBase) are left untouched.
+static void skip_distances(std::vector<uint16_t>& grid, const int dims[3]) {
+  const int Nx = dims[0], Ny = dims[1], Nz = dims[2];
+  const size_t N = (size_t)Nx * Ny * Nz;
+  std::vector<uint8_t> dist(N);
+  for (size_t v = 0; v < N; ++v) dist[v] = grid[v] < kEmptyBase ? 0 : 255;
+  auto relax = [&](int z, int y, int x, int sgn) {
+    // 13 neighbours that precede (sgn = -1) or follow (sgn = +1) the voxel in raster order
+    uint8_t& c = dist[((size_t)z * Ny + y) * Nx + x];
+    int m = c;
+    if (m == 0) return;
+    for (int dz = 0; dz <= 1; ++dz) {
+      const int z2 = z + sgn * dz;
+      if (z2 < 0 || z2 >= Nz) continue;
+      for (int dy = (dz ? -1 : 0); dy <= 1; ++dy) {
+        const int y2 = y + sgn * dy;
+        if (y2 < 0 || y2 >= Ny) continue;
+        for (int dx = ((dz || dy) ? -1 : 1); dx <= 1; ++dx) {
+          const int x2 = x + sgn * dx;
+          if (x2 < 0 || x2 >= Nx) continue;
+          const int nb = dist[((size_t)z2 * Ny + y2) * Nx + x2] + 1;
+          if (nb < m) m = nb;
+        }
+      }
+    }
+    c = (uint8_t)m;
+  };
+  // forward scan uses the neighbours already visited (sgn = -1), backward scan the others
+  for (int z = 0; z < Nz; ++z)
+    for (int y = 0; y < Ny; ++y)
+      for (int x = 0; x < Nx; ++x) relax(z, y, x, -1);
+  for (int z = Nz - 1; z >= 0; --z)
+    for (int y = Ny - 1; y >= 0; --y)
+      for (int x = Nx - 1; x >= 0; --x) relax(z, y, x, +1);
+  for (size_t v = 0; v < N; ++v)
+    if (grid[v] >= kEmptyBase) grid[v] = (uint16_t)(kEmptyBase | dist[v]);
+}
 
 extern "C" {
 
@@ -147,6 +187,7 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
     g.box_min[a] = desc->box_min[a];
     volatile float ext = desc->box_max[a] - desc->box_min[a];
     g.vs[a] = ext / (float)desc->dims[a];
+    g.inv_vs[a] = 1.0f / g.vs[a];
   }
   g.K = desc->samples_per_voxel;
   g.Kf = (float)g.K;
@@ -167,7 +208,7 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
     hi.assign((size_t)n * 3, -1);
   } catch (const std::bad_alloc&) { return R360_ERR_OOM; }
   for (long long v = 0; v < N; ++v) {
-    if (occupancy[v] < desc->occ_threshold) { grid[(size_t)v] = (uint16_t)kEmptyVoxel; continue; }
+    if (occupancy[v] < desc->occ_threshold) { grid[(size_t)v] = (uint16_t)(kEmptyBase | 0xFFu); continue; }
     int k = voxel_subfield[v];
     if (k < 0 || k >= n) return R360_ERR_BAD_LABEL;
     grid[(size_t)v] = (uint16_t)k;
@@ -178,6 +219,7 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
       if (idx[a] > hi[(size_t)k * 3 + a]) hi[(size_t)k * 3 + a] = idx[a];
     }
   }
+  skip_distances(grid, g.dims);
   for (long long i = 0; i < (long long)n * src.total; ++i)
     if (!std::isfinite(weights[i])) return R360_ERR_NONFINITE;
   std::vector<SubfieldFrame> frames((size_t)n);

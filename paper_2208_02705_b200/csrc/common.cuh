@@ -6,7 +6,12 @@
 
 namespace r360 {
 
-constexpr uint32_t kEmptyVoxel = 0xFFFFu;   // fused occupancy+label grid: 0xFFFF = empty
+// Fused occupancy + label + skip-distance grid (uint16 per voxel):
+//   value <  kEmptyBase : occupied, the value is the subfield label
+//   value >= kEmptyBase : empty, low byte = D = min(255, chessboard distance in voxels to the nearest
+//                         occupied voxel) >= 1, i.e. the cube of half-size D-1 around the voxel is empty
+constexpr uint32_t kEmptyBase = 0xFF00u;
+constexpr int kMaxSubfields = 0xFF00;
 constexpr int kTileRows = 128;              // rows (samples) per MLP tile
 constexpr float kParallelEps = 7.888609052210118e-31f;  // 2^-100: |d_a| below = axis-parallel (reading C1)
 
@@ -15,6 +20,7 @@ struct GridParams {
   int dims[3];
   float box_min[3];
   float vs[3];           // voxel size per axis: (box_max - box_min) / dims, binary32 (reading C)
+  float inv_vs[3];       // 1 / vs: only for index GUESSES that are then verified against the planes
   int K;                 // samples per occupied voxel crossed (reading D)
   float Kf;
 };
@@ -80,18 +86,24 @@ __device__ __forceinline__ float plane(const GridParams& g, int a, int k) {
 }
 
 // ---------------------------------------------------------------------------------------
-// Voxel walk (readings C1-C4) as a resumable state machine.  next() advances to the next
-// OCCUPIED voxel the ray crosses (t_in < t_out, strict), front to back, and returns false when
-// the ray has left the grid.  Distances always come from the voxel index through t_at(); only
-// the axis that stepped is recomputed, and the new near distance of that axis is the old far
-// distance (same formula, same index => same bits as recomputing it).
+// Voxel walk (readings C1-C4) with exact empty-space skipping.  next() advances to the next OCCUPIED
+// voxel the ray crosses (t_in < t_out, strict), front to back, and returns false when the ray has
+// left the grid.
+//
+// Reading C5: the crossed set is a per-voxel predicate, max(t0, max_a tn_a(i)) < min_a tf_a(i), with
+// every distance computed from the voxel index through t_at(); it does not depend on the path taken.
+// So from an empty voxel whose skip distance is D the walk leaves the whole empty cube of half-size
+// r = D-1 at once: the exit distance `to` is the smallest far-plane distance of the CUBE, the axis of
+// the minimum steps to the voxel behind that plane, and on the other two axes the new index is the
+// first one (along the ray) whose far plane lies beyond `to` -- found from a position guess and then
+// verified against the planes themselves, so no rounding of the guess can change the result.
+// The entry distance of the next voxel is max(t0, to, its near planes), which is exactly the
+// oracle's max(t0, tn_x, tn_y, tn_z); for a plain one-voxel step this reduces to max(ti, to).
 struct Walker {
-  float o[3], inv[3];
-  float tn[3], tf[3];
-  float t0;
+  float o[3], d[3], inv[3];
+  float t0, ti;     // clip distance; entry distance of the current voxel
   int idx[3];
-  int v;            // linear voxel index
-  bool neg[3];
+  bool neg[3], par[3];
   bool alive;
 
   __device__ __forceinline__ float t_at(const GridParams& g, int a, int k) const {
@@ -99,11 +111,11 @@ struct Walker {
   }
 
   __device__ __forceinline__ void init(const GridParams& g, const Ray& ray) {
-    bool par[3];
     alive = true;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       o[a] = ray.o[a];
+      d[a] = ray.d[a];
       par[a] = fabsf(ray.d[a]) < kParallelEps;
       neg[a] = ray.d[a] < 0.0f;
       inv[a] = par[a] ? 0.0f : __fdiv_rn(1.0f, ray.d[a]);
@@ -124,51 +136,77 @@ struct Walker {
       }
     }
     if (!(t0 < t1)) alive = false;
-    // C3: start voxel
+    // C3: start voxel; C4: its entry distance
+    ti = t0;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       float pa = __fmaf_rn(t0, ray.d[a], o[a]);
       float f = floorf(__fdiv_rn(__fsub_rn(pa, g.box_min[a]), g.vs[a]));
       int N = g.dims[a];
       idx[a] = (f < 0.0f) ? 0 : ((f > (float)(N - 1)) ? N - 1 : (int)f);
-      if (par[a]) {
-        tn[a] = __int_as_float(0xff800000);
-        tf[a] = __int_as_float(0x7f800000);
-      } else {
-        tn[a] = t_at(g, a, idx[a] + (neg[a] ? 1 : 0));
-        tf[a] = t_at(g, a, idx[a] + (neg[a] ? 0 : 1));
-      }
+      if (!par[a]) ti = fmaxf(ti, t_at(g, a, idx[a] + (neg[a] ? 1 : 0)));
     }
-    v = (idx[2] * g.dims[1] + idx[1]) * g.dims[0] + idx[0];
   }
 
-  // C4.  On true: lab = subfield label of the voxel, [t_in, t_out] its crossing interval.
+  // On true: lab = subfield label of the voxel, [t_in, t_out] its crossing interval.
   __device__ __forceinline__ bool next(const GridParams& g, const uint16_t* __restrict__ grid,
                                        uint32_t& lab, float& t_in, float& t_out) {
+    const float inf = __int_as_float(0x7f800000);
     while (alive) {
-      float ti = fmaxf(fmaxf(t0, tn[0]), fmaxf(tn[1], tn[2]));
+      const uint32_t l = __ldg(grid + (idx[2] * g.dims[1] + idx[1]) * g.dims[0] + idx[0]);
+      const bool empty = l >= kEmptyBase;
+      const int r = empty ? (int)(l & 0xFFu) - 1 : 0;     // half-size of the empty cube (0: this voxel only)
+      // far planes of the cube [idx - r, idx + r], clamped to the grid
+      int kx[3];
+      float tf[3];
+#pragma unroll
+      for (int a = 0; a < 3; ++a) {
+        kx[a] = neg[a] ? max(idx[a] - r, 0) : min(idx[a] + r + 1, g.dims[a]);
+        tf[a] = par[a] ? inf : t_at(g, a, kx[a]);
+      }
       int amin = 2;
       float to = tf[2];
       if (tf[1] <= to) { to = tf[1]; amin = 1; }
       if (tf[0] <= to) { to = tf[0]; amin = 0; }   // ties -> lowest axis
-      bool hit = false;
-      if (ti < to) {
-        uint32_t l = __ldg(grid + v);
-        if (l != kEmptyVoxel) { hit = true; lab = l; t_in = ti; t_out = to; }
-      }
-      // advance along amin (selects instead of dynamic register indexing)
-      int stride = 1;
+      const bool hit = !empty && ti < to;
+      if (hit) { lab = l; t_in = ti; t_out = to; }
+      // step across the far plane of the axis of the minimum
 #pragma unroll
       for (int a = 0; a < 3; ++a) {
         if (a == amin) {
-          int s = neg[a] ? -1 : 1;
-          idx[a] += s;
-          v += s * stride;
-          tn[a] = tf[a];
-          tf[a] = t_at(g, a, idx[a] + (neg[a] ? 0 : 1));
-          if (idx[a] < 0 || idx[a] >= g.dims[a]) alive = false;
+          idx[a] = neg[a] ? kx[a] - 1 : kx[a];
+          if ((unsigned)idx[a] >= (unsigned)g.dims[a]) alive = false;
         }
-        stride *= g.dims[a];
+      }
+      if (r > 0) {
+        // left a cube: re-derive the index on the other axes from the planes
+        float tin = fmaxf(t0, to);
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+          if (a != amin && !par[a] && alive) {
+            const int lo = max(idx[a] - r, 0), hi = min(idx[a] + r, g.dims[a] - 1);
+            const int first = neg[a] ? hi : lo, step = neg[a] ? -1 : 1, off = neg[a] ? 0 : 1;
+            const float p = __fmaf_rn(to, d[a], o[a]);
+            int gi = __float2int_rd((p - g.box_min[a]) * g.inv_vs[a]);     // guess, verified below
+            gi = min(max(gi, lo), hi);
+            // forward: the far plane of gi must lie beyond `to`
+            while (!(t_at(g, a, gi + off) > to)) {
+              gi += step;
+              if ((unsigned)gi >= (unsigned)g.dims[a]) { alive = false; break; }
+            }
+            // backward: no earlier index of the cube may qualify; tn = near plane of gi
+            float tn = t_at(g, a, gi - step + off);
+            while (gi != first && tn > to) {
+              gi -= step;
+              tn = t_at(g, a, gi - step + off);
+            }
+            idx[a] = gi;
+            tin = fmaxf(tin, tn);
+          }
+        }
+        ti = tin;
+      } else {
+        ti = fmaxf(ti, to);
       }
       if (hit) return true;
     }

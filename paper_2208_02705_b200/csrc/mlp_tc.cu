@@ -337,6 +337,15 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
       rec = __ldg(b.recs + seg0 + sidx);
       rd = __ldg(b.rec_dir + seg0 + sidx);                   // direction, pose
     }
+    if (j == 0) {
+      // hide DRAM latency without registers: this tile's direction block (read after trunk-1 is
+      // issued) and the next tile's records go to L2 now
+      if (active) prefetch_l2(b.dirblk + (size_t)rec.x * 4);
+      if (seg0 + spt + sidx < k_seg_end) {
+        prefetch_l2(b.recs + seg0 + spt + sidx);
+        prefetch_l2(b.rec_dir + seg0 + spt + sidx);
+      }
+    }
     const float* P = f.poses + rd.w * 12;
     const float t = __fmaf_rn(jf, __uint_as_float(rec.z), __uint_as_float(rec.y));   // reading D
     float q[3];                                              // reading A3

@@ -13,7 +13,7 @@ struct r360_scene {
   int n_sms = 148;
   int segs_per_tile = 16;
   // scene-constant device data
-  uint16_t* d_grid = nullptr;               // fused occupancy + label, 0xFFFF = empty
+  uint16_t* d_grid = nullptr;               // fused occupancy + label + skip distance (common.cuh)
   r360::SubfieldFrame* d_frames = nullptr;  // [n]
   float* d_wt = nullptr;                    // [n * lay.total] fp32, transposed + padded
   void* d_wpack = nullptr;                  // [n * wpack_stride] bf16 operand tiles + fp32 biases

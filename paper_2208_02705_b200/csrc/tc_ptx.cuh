@@ -57,6 +57,11 @@ __device__ __forceinline__ bool elect_one() {
   return pred != 0;
 }
 
+// L2 prefetch of the line holding p (no register, no scoreboard)
+__device__ __forceinline__ void prefetch_l2(const void* p) {
+  asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
 // ---- TMA 1-D bulk copy global -> shared, completes on an mbarrier (async proxy) ----------
 __device__ __forceinline__ void bulk_g2s(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
