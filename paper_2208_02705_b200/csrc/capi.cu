@@ -159,6 +159,7 @@ void r360_scene_destroy(r360_scene* sc) {
   cudaFree(sc->buf.tile_start); cudaFree(sc->buf.totals);
   cudaFree(sc->buf.seg_tin); cudaFree(sc->buf.seg_dt); cudaFree(sc->buf.recs); cudaFree(sc->buf.out);
   cudaFree(sc->d_dirblk); cudaFree(sc->d_rec_dir);
+  cudaFree(sc->buf.hit_t); cudaFree(sc->buf.hit_lab);
   cudaFree(sc->d_stage_rgb); cudaFree(sc->d_stage_depth);
   if (sc->h_totals) cudaFreeHost(sc->h_totals);
   for (auto& ce : sc->events)

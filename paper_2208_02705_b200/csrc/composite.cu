@@ -21,18 +21,28 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __res
       const float t_in = b.seg_tin[off + s];
       const float dt = b.seg_dt[off + s];
       const float4* o = b.out + (size_t)(off + s) * K;
-      for (int j = 0; j < K; ++j) {
-        const float4 v = __ldcs(o + j);
-        const float t = __fmaf_rn((float)j + 0.5f, dt, t_in);
-        const float alpha = 1.0f - expf(-v.x * dt);
-        const float w = T * alpha;
-        C0 = fmaf(w, v.y, C0);
-        C1 = fmaf(w, v.z, C1);
-        C2 = fmaf(w, v.w, C2);
-        D = fmaf(w, t, D);
-        T = T * (1.0f - alpha);
-        ++used;
-        if (T < tau) { done = true; break; }
+      // the K samples of a segment are K consecutive float4: fetch them eight at a time, back to back,
+      // so that every 128-byte line is requested once, whole, and not re-fetched after an L1 eviction
+      for (int j0 = 0; j0 < K && !done; j0 += 8) {
+        float4 v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u)
+          if (j0 + u < K) v[u] = __ldcs(o + j0 + u);
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+          if (j0 + u < K && !done) {
+            const float t = __fmaf_rn((float)(j0 + u) + 0.5f, dt, t_in);
+            const float alpha = 1.0f - expf(-v[u].x * dt);
+            const float w = T * alpha;
+            C0 = fmaf(w, v[u].y, C0);
+            C1 = fmaf(w, v[u].z, C1);
+            C2 = fmaf(w, v[u].w, C2);
+            D = fmaf(w, t, D);
+            T = T * (1.0f - alpha);
+            ++used;
+            if (T < tau) done = true;
+          }
+        }
       }
     }
     const size_t gr = (size_t)(f.ray0 + (long long)r);

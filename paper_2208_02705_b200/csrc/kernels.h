@@ -46,12 +46,16 @@ struct ChunkBuffers {
   float* seg_dt;         // [G] ray-major
   SegRec* recs;          // [G] binned by subfield
   float4* out;           // [G*K] (sigma, r, g, b) per sample, ray-major
+  // first kHitCap hits of every ray, kept by k_count so that k_emit re-walks only the rays with more
+  float2* hit_t;         // [kHitCap][n_rays] (t_in, delta)
+  uint16_t* hit_lab;     // [kHitCap][n_rays]
   // tensor path only (null otherwise):
   uint4* dirblk;         // [n_rays*4] per ray: [1, 1, F(d), 0..] as 32 bf16 (pe.cuh)
   uint4* rec_dir;        // [G] binned like recs: (d.x, d.y, d.z, pose index)
 };
 
 constexpr int kSamplerThreads = 256;
+constexpr int kHitCap = 16;
 
 void launch_count(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
                   int n_bins, cudaStream_t s);

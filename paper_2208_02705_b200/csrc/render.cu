@@ -90,6 +90,8 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
   if ((st = grow(sc->buf.ray_cnt, sc->ray_cnt_cap, f.n_rays, 1, 1)) != R360_OK) return st;
   if ((st = grow(sc->buf.ray_off, sc->ray_off_cap, f.n_rays, 1, 1)) != R360_OK) return st;
   if ((st = grow(sc->buf.block_sum, sc->blocks_cap, n_blocks, 1, 1)) != R360_OK) return st;
+  if ((st = grow(sc->buf.hit_t, sc->hit_t_cap, (size_t)f.n_rays * kHitCap, 1, 1)) != R360_OK) return st;
+  if ((st = grow(sc->buf.hit_lab, sc->hit_lab_cap, (size_t)f.n_rays * kHitCap, 1, 1)) != R360_OK) return st;
   if (sc->precision == 1) {            // tensor path: per-ray records (direction + packed F(d))
     if ((st = grow(sc->d_dirblk, sc->dirblk_cap, (size_t)f.n_rays * 4, 1, 1)) != R360_OK) return st;
     sc->buf.dirblk = sc->d_dirblk;

@@ -72,6 +72,12 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
     bool hit = w.next(g, grid, lab, t_in, t_out);
     unsigned m = __ballot_sync(0xffffffffu, hit);
     if (hit) {
+      if (cnt < kHitCap) {
+        // reading D: delta = (t_out - t_in) / K, one subtract, one divide
+        const size_t h = (size_t)cnt * f.n_rays + r;
+        b.hit_t[h] = make_float2(t_in, __fdiv_rn(__fsub_rn(t_out, t_in), g.Kf));
+        b.hit_lab[h] = (uint16_t)lab;
+      }
       ++cnt;
       unsigned peers = __match_any_sync(m, lab);
       if ((peers & lanemask_lt()) == 0) {
@@ -163,23 +169,41 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
   const bool valid = r < f.n_rays;
   Walker w;
   w.alive = false;
-  uint32_t slot = 0;
+  uint32_t slot = 0, cnt = 0, h = 0;
   uint4 dir = make_uint4(0, 0, 0, 0);
+  bool replay = false;
   if (valid) {
     const Ray ray = make_ray(f, r);
-    w.init(g, ray);
     dir = make_uint4(__float_as_uint(ray.d[0]), __float_as_uint(ray.d[1]), __float_as_uint(ray.d[2]), ray.pose);
     slot = b.block_sum[blockIdx.x] + b.ray_off[r];
     b.ray_off[r] = slot;                 // now the global ray-major offset
+    cnt = b.ray_cnt[r];
+    replay = cnt <= kHitCap;             // every hit of this ray is in the hit buffer
+    if (!replay) w.init(g, ray);         // otherwise walk again
   }
-  while (__any_sync(0xffffffffu, w.alive)) {
+  bool more = replay ? cnt > 0 : w.alive;
+  while (__any_sync(0xffffffffu, more)) {
     uint32_t lab = 0;
-    float t_in = 0.f, t_out = 0.f;
-    bool hit = w.next(g, grid, lab, t_in, t_out);
+    float t_in = 0.f, dt = 0.f;
+    bool hit = false;
+    if (replay) {
+      if (h < cnt) {
+        const size_t i = (size_t)h * f.n_rays + r;
+        const float2 td = b.hit_t[i];
+        t_in = td.x; dt = td.y;
+        lab = b.hit_lab[i];
+        hit = true;
+        ++h;
+      }
+      more = h < cnt;
+    } else {
+      float t_out = 0.f;
+      hit = w.next(g, grid, lab, t_in, t_out);
+      if (hit) dt = __fdiv_rn(__fsub_rn(t_out, t_in), g.Kf);    // reading D
+      more = w.alive;
+    }
     unsigned m = __ballot_sync(0xffffffffu, hit);
     if (hit) {
-      // reading D: delta = (t_out - t_in) / K, one subtract, one divide
-      float dt = __fdiv_rn(__fsub_rn(t_out, t_in), g.Kf);
       unsigned peers = __match_any_sync(m, lab);
       int leader = __ffs(peers) - 1;
       uint32_t base = 0;
