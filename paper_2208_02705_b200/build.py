@@ -24,7 +24,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     deps = srcs + [os.path.normpath(os.path.join(CSRC, h)) for h in HEADERS]
     if not force and os.path.exists(SO) and os.path.getmtime(SO) >= max(os.path.getmtime(d) for d in deps):
         return SO
-    cmd = [_nvcc(), *NVCC_FLAGS, "-o", SO, *srcs]
+    cmd = [_nvcc(), *NVCC_FLAGS, *os.environ.get("R360_NVCC_FLAGS", "").split(), "-o", SO, *srcs]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.check_call(cmd)

@@ -38,3 +38,19 @@ def check_image(gpu_rgb, gpu_depth, ref, tol, amb_band=1e-3, depth_tol=None):
         assert np.all((g_rgb[amb] >= lo) & (g_rgb[amb] <= hi))
         assert np.all((g_d[amb] >= ref["depth"][amb] - depth_tol) & (g_d[amb] <= ref["depth_full"][amb] + depth_tol))
     return max_rgb, max_d, int(amb.sum())
+
+
+def ray_major_index(counts, offsets):
+    """Gather index that lists every ray's samples, rays in ray-major order.
+
+    The order of the rays inside the sample buffers is free (the bit-exact
+    contract covers, per ray, the count and the sequence of (t, subfield)); what must hold is that the
+    per-ray ranges [offset, offset + count) are disjoint and cover [0, total).  Returns the index and
+    checks exactly that."""
+    counts = np.asarray(counts, np.int64).reshape(-1)
+    offsets = np.asarray(offsets, np.int64).reshape(-1)
+    total = int(counts.sum())
+    first = np.repeat(np.cumsum(counts) - counts, counts)       # ray-major start of each sample's ray
+    idx = np.repeat(offsets, counts) + (np.arange(total, dtype=np.int64) - first)
+    assert np.array_equal(np.sort(idx), np.arange(total, dtype=np.int64)), "per-ray ranges overlap or leave gaps"
+    return idx

@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 from conftest import get_scene
-from gpu_util import check_image, with_density_bias
+from gpu_util import check_image, ray_major_index, with_density_bias
 
 pytestmark = pytest.mark.gpu
 F = np.float32
@@ -31,9 +31,9 @@ def _cmp_samples(r360, oracle, sc, pose, W, H, **override):
     oc, ot, osid = ora.samples_rows(pose, W, H)
     counts, offsets = counts.cpu().numpy().view(np.uint32), offsets.cpu().numpy().view(np.uint32)
     assert np.array_equal(counts, oc)                                           # bit-exact counts
-    assert np.array_equal(offsets.astype(np.int64), np.concatenate([[0], np.cumsum(oc.astype(np.int64))[:-1]]))
-    assert np.array_equal(t.cpu().numpy().view(np.uint32), ot.view(np.uint32))  # bit-exact distances
-    assert np.array_equal(sid.cpu().numpy(), osid)                              # exact subfield ids
+    idx = ray_major_index(counts, offsets)                                      # valid layout, any ray order
+    assert np.array_equal(t.cpu().numpy().view(np.uint32)[idx], ot.view(np.uint32))  # bit-exact distances
+    assert np.array_equal(sid.cpu().numpy()[idx], osid)                         # exact subfield ids
     gpu.close()
     return int(oc.sum())
 
@@ -182,12 +182,15 @@ def test_full_size_config3_sampled(r360, oracle):
     check_image(g_rgb, g_d, ref, 1e-4)
     counts, offsets, t, sid = gpu.debug_samples(sc.poses[0], sc.W, sc.H)
     counts = counts.cpu().numpy().view(np.uint32).reshape(sc.H, sc.W)
+    offsets = offsets.cpu().numpy().view(np.uint32).reshape(sc.H, sc.W)
+    ray_major_index(counts, offsets)
+    t_np, sid_np = t.cpu().numpy().view(np.uint32), sid.cpu().numpy()
     assert int(counts.sum()) == st.samples_emitted
     assert np.array_equal(counts[py, px], ref["n_emitted"])
     for row in (0, 511, 1023):
         oc, ot, osid = ora.samples_rows(sc.poses[0], sc.W, sc.H, row, row + 1)
         assert np.array_equal(counts[row], oc)
-        o0 = int(offsets[row * sc.W].item())
-        n = int(oc.sum())
-        assert np.array_equal(t[o0:o0 + n].cpu().numpy().view(np.uint32), ot.view(np.uint32))
-        assert np.array_equal(sid[o0:o0 + n].cpu().numpy(), osid)
+        oc64 = oc.astype(np.int64)
+        idx = np.repeat(offsets[row].astype(np.int64), oc64) + (np.arange(int(oc64.sum())) - np.repeat(np.cumsum(oc64) - oc64, oc64))
+        assert np.array_equal(t_np[idx], ot.view(np.uint32))
+        assert np.array_equal(sid_np[idx], osid)
