@@ -26,12 +26,14 @@ def _t_max(sc):
     return float(np.linalg.norm(np.array(sc.box_max) - np.array(sc.box_min)))
 
 
-def _cmp(r360, oracle, sc, weights=None, amb_band=0.2, px=None, py=None, tol=TOL, **desc_over):
+def _cmp(r360, oracle, sc, weights=None, amb_band=0.2, px=None, py=None, tol=TOL, precision="bf16", pose=None,
+         **desc_over):
     over = dict(desc_over)
     if weights is not None:
         over["weights"] = weights
     gpu = r360.scene_from(sc, **over)
-    gpu.set_precision("bf16")
+    gpu.set_precision(precision)
+    pose = sc.poses[0] if pose is None else pose
     okw = dict(dims=sc.dims, box_min=sc.box_min, box_max=sc.box_max, n_subfields=sc.n_subfields,
                hidden_width=sc.hidden_width, n_hidden=sc.n_hidden, pe_pos_levels=sc.pe_pos_levels,
                pe_dir_levels=sc.pe_dir_levels, samples_per_voxel=sc.samples_per_voxel,
@@ -40,16 +42,17 @@ def _cmp(r360, oracle, sc, weights=None, amb_band=0.2, px=None, py=None, tol=TOL
                weights=sc.weights if weights is None else weights)
     okw.update(desc_over)
     ora = oracle.scene(**okw)
-    rgb, depth = gpu.render(sc.poses[0], sc.W, sc.H)
+    rgb, depth = gpu.render(pose, sc.W, sc.H)
     st = gpu.stats()
     rgb, depth = rgb.cpu().numpy(), depth.cpu().numpy()
     if px is None:
-        ref = ora.render_rows(sc.poses[0], sc.W, sc.H)
+        ref = ora.render_rows(pose, sc.W, sc.H)
         assert st.samples_emitted == int(ref["n_emitted"].sum())
     else:
-        ref = ora.render_pixels(sc.poses[0], sc.W, sc.H, px, py)
+        ref = ora.render_pixels(pose, sc.W, sc.H, px, py)
         rgb, depth = rgb[py, px], depth[py, px]
-    res = check_image(rgb, depth, ref, tol, amb_band=amb_band, depth_tol=tol * _t_max(sc))
+    depth_tol = tol * _t_max(sc) if precision == "bf16" else tol
+    res = check_image(rgb, depth, ref, tol, amb_band=amb_band, depth_tol=depth_tol)
     gpu.close()
     return res
 
@@ -112,7 +115,8 @@ def test_bf16_refused_for_other_pe_sizes(r360, scene1):
     P = mlp_param_count(32, 2, 6, 4)
     gpu = r360.scene_from(sc, weights=np.zeros(sc.n_subfields * P, F), pe_pos_levels=6)
     with pytest.raises(r360.R360Error):
-        gpu.set_precision("bf16")
+        gpu.set_precision(precision)
+    pose = sc.poses[0] if pose is None else pose
 
 
 def test_full_size_config3_bf16_sampled(r360, oracle):
@@ -122,3 +126,52 @@ def test_full_size_config3_bf16_sampled(r360, oracle):
     py = rng.integers(0, sc.H, 3000).astype(np.int32)
     e_rgb, e_d, n_amb = _cmp(r360, oracle, sc, px=px, py=py)
     print("config3 bf16 sampled max rgb err", e_rgb, "depth", e_d)
+
+
+@pytest.mark.parametrize("n_hidden", [2, 3])
+def test_render_bf16_random_biases(r360, oracle, n_hidden):
+    # every bias path of the tensor kernel: the single bf16 bias row of the first layer, the hi/lo rows of
+    # the hidden layers, the bias of the folded feature+colour layer, the fp32 biases of the two heads
+    from scenegen import mlp_param_count, weight_layout
+    sc = get_scene(1)
+    rng = np.random.default_rng(23 + n_hidden)
+    parts = []
+    for name, fo, fi in weight_layout(32, n_hidden):
+        a = np.sqrt(6.0 / (fi + fo))
+        parts.append(rng.uniform(-a, a, (sc.n_subfields, fo * fi)))
+        b = rng.uniform(-0.5, 0.5, (sc.n_subfields, fo))
+        if name == "density":
+            b += 1.0
+        parts.append(b)
+    w = np.concatenate(parts, 1).astype(F).reshape(-1)
+    assert w.size == sc.n_subfields * mlp_param_count(32, n_hidden)
+    e_rgb, e_d, _ = _cmp(r360, oracle, sc, weights=w, n_hidden=n_hidden)
+    print("random biases, n_hidden", n_hidden, "bf16 max rgb err", e_rgb)
+    _cmp(r360, oracle, sc, weights=w, n_hidden=n_hidden, precision="fp32", tol=1e-4, amb_band=1e-3)
+
+
+def _sampled(sc, n, seed):
+    rng = np.random.default_rng(seed)
+    return rng.integers(0, sc.W, n).astype(np.int32), rng.integers(0, sc.H, n).astype(np.int32)
+
+
+def test_full_size_config5_sampled(r360, oracle):
+    """BASELINE.json config 5 (load imbalance, density bias -2, ~290 samples per ray) at full size, both paths,
+    on pixels the oracle renders one by one."""
+    sc = get_scene(5)
+    px, py = _sampled(sc, 1200, 7)
+    e_rgb, e_d, _ = _cmp(r360, oracle, sc, px=px, py=py)
+    print("config5 bf16 sampled max rgb err", e_rgb, "depth", e_d)
+    e_rgb, e_d, _ = _cmp(r360, oracle, sc, px=px, py=py, precision="fp32", tol=1e-4, amb_band=1e-3)
+    print("config5 fp32 sampled max rgb err", e_rgb, "depth", e_d)
+
+
+def test_full_size_config4_one_pose_sampled(r360, oracle):
+    """BASELINE.json config 4 (width 64, K = 12, 4096 subfields, 4096x2048) -- one pose of the batch of 8, in two
+    ray chunks, both paths, on sampled pixels."""
+    sc = get_scene(4)
+    px, py = _sampled(sc, 1200, 9)
+    e_rgb, e_d, _ = _cmp(r360, oracle, sc, px=px, py=py, pose=sc.poses[3])
+    print("config4 bf16 sampled max rgb err", e_rgb, "depth", e_d)
+    e_rgb, e_d, _ = _cmp(r360, oracle, sc, px=px, py=py, pose=sc.poses[3], precision="fp32", tol=1e-4, amb_band=1e-3)
+    print("config4 fp32 sampled max rgb err", e_rgb, "depth", e_d)
