@@ -35,6 +35,22 @@ def flop_per_sample(width, n_hidden, pe_p=63, pe_d=27):
     return 2 * macs
 
 
+def executed_flop_per_sample(width, n_hidden, pe_p=63, pe_d=27):
+    """Unpadded contraction the tensor kernel actually runs: the feature layer (no activation) is folded
+    into the colour layer on the host, so its width x width product is not evaluated per sample."""
+    return flop_per_sample(width, n_hidden, pe_p, pe_d) - 2 * width * width
+
+
+def ncu_traffic(kernel):
+    """DRAM bytes (read + write) of one launch of `kernel` on this workload, from the committed ncu --set full
+    capture (profiles/traffic.json, written by hand from the capture named there); None if not recorded."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p)).get(kernel)
+    except (OSError, ValueError):
+        return None
+
+
 def measured_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -146,6 +162,49 @@ def workload_config(sc, args, precision):
             "l2": "explicit L2 flush (512 MiB memset) between timed iterations, outside the CUDA events"}
 
 
+def time_config(r360, config, precision, steps=5, warmup=3):
+    """Short device-timed run of another BASELINE.json config (all its poses in one batch call)."""
+    import torch
+    from scenegen import make_scene
+    sc = make_scene(config)
+    scene = r360.scene_from(sc)
+    scene.set_precision(precision)
+    scene.use_current_torch_stream()
+    B, W, H = len(sc.poses), sc.W, sc.H
+    poses = np.ascontiguousarray(np.stack([np.asarray(p, np.float32) for p in sc.poses]))
+    rgb = torch.empty((B, H, W, 3), dtype=torch.float32, device="cuda")
+    depth = torch.empty((B, H, W), dtype=torch.float32, device="cuda")
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+    for _ in range(warmup):
+        scene.render_batch(poses, W, H, rgb, depth)
+    torch.cuda.synchronize()
+    ms, ms_mlp = 0.0, 0.0
+    for _ in range(steps):
+        flush.zero_()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        scene.render_batch(poses, W, H, rgb, depth)
+        e1.record()
+        st = scene.stats()
+        ms += e0.elapsed_time(e1)
+        ms_mlp += st.ms_mlp
+    ms /= steps
+    ms_mlp /= steps
+    fl = flop_per_sample(sc.hidden_width, sc.n_hidden)
+    peaks = measured_peaks()
+    out = {"config": config, "name": sc.name, "image": [W, H], "poses": B, "n_subfields": sc.n_subfields,
+           "mlp": [sc.n_hidden, sc.hidden_width], "K": sc.samples_per_voxel, "precision": precision,
+           "ms_per_step": ms, "rays_per_s": B * W * H / (ms * 1e-3), "fps": B * 1e3 / ms,
+           "samples_per_step": int(st.samples_emitted), "mlp_samples_per_s": st.samples_emitted / (ms_mlp * 1e-3),
+           "ms_mlp": ms_mlp, "chunks": int(st.chunks)}
+    if precision == "bf16":
+        out["mlp_frac_of_bf16_sustained"] = st.samples_emitted * fl / (ms_mlp * 1e-3) / 1e12 / peaks["bf16_sustained"]
+    scene.close()
+    del rgb, depth, flush
+    torch.cuda.empty_cache()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -156,6 +215,8 @@ def main():
     ap.add_argument("--precision", default="auto", choices=["auto", "fp32", "bf16"])
     ap.add_argument("--ref-row-stride", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--all-configs", action="store_true",
+                    help="also time BASELINE.json's other configs (short runs) and add them as other_configs")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -257,6 +318,10 @@ def main():
                     "unit": "TFLOP/s", "frac": ach / ALU_PEAK_TFLOPS, "traffic": None,
                     "peak_source": "derived: 148 SM x 128 FMA/clk x 2 x 1.965 GHz"}
         roof["flop_per_sample"] = fl
+        if precision == "bf16" and args.config == 3:
+            roof["traffic"] = ncu_traffic("k_mlp_tc")
+        if precision == "bf16":
+            roof["executed_flop_per_sample"] = executed_flop_per_sample(sc.hidden_width, sc.n_hidden)
         roof["samples_per_launch"] = int(samples)
         roof["ms_per_launch"] = ms_mlp
         line = {"metric": "rays_per_second_equirect_render", "value": value, "unit": "rays/s", "n_gpus": world,
@@ -270,6 +335,10 @@ def main():
                 "e2e": {"value": e2e_value, "unit": "rays/s", "h2d_bytes_per_step": 48 * world,
                         "d2h_bytes_per_step": W * H * 16 * world},
                 "gpu_launches": int(launches)}
+        if args.all_configs:
+            scene.close()
+            del rgb, depth
+            line["other_configs"] = [time_config(r360, c, precision) for c in (1, 2, 4, 5) if c != args.config]
         if not args.no_cpu_baseline:
             cb = oracle_sample(sc, args.ref_row_stride)
             line["cpu_baseline"] = {"value": cb["rays_per_s"], "unit": "rays/s", "cores": cb["cores"],
