@@ -115,8 +115,7 @@ def test_bf16_refused_for_other_pe_sizes(r360, scene1):
     P = mlp_param_count(32, 2, 6, 4)
     gpu = r360.scene_from(sc, weights=np.zeros(sc.n_subfields * P, F), pe_pos_levels=6)
     with pytest.raises(r360.R360Error):
-        gpu.set_precision(precision)
-    pose = sc.poses[0] if pose is None else pose
+        gpu.set_precision("bf16")
 
 
 def test_full_size_config3_bf16_sampled(r360, oracle):
