@@ -160,6 +160,7 @@ void r360_scene_destroy(r360_scene* sc) {
   cudaFree(sc->buf.seg_tin); cudaFree(sc->buf.seg_dt); cudaFree(sc->buf.recs); cudaFree(sc->buf.out);
   cudaFree(sc->d_dirblk); cudaFree(sc->d_rec_dir);
   cudaFree(sc->buf.hit_t); cudaFree(sc->buf.hit_lab);
+  cudaFree(sc->buf.bin_ovf); cudaFree(sc->buf.blk_list); cudaFree(sc->buf.blk_list_n);
   cudaFree(sc->d_stage_rgb); cudaFree(sc->d_stage_depth);
   if (sc->h_totals) cudaFreeHost(sc->h_totals);
   for (auto& ce : sc->events)
@@ -278,6 +279,7 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
     R360_CUDA(cudaMemcpy(sc->d_wpack, wpack.data(), wpack.size(), cudaMemcpyHostToDevice));
   }
   R360_CUDA(cudaMalloc(&sc->buf.bin_cnt, (size_t)n * 4));
+  R360_CUDA(cudaMalloc(&sc->buf.bin_ovf, (size_t)n * 4));
   R360_CUDA(cudaMalloc(&sc->buf.bin_start, (size_t)(n + 1) * 4));
   R360_CUDA(cudaMalloc(&sc->buf.bin_cursor, (size_t)n * 4));
   R360_CUDA(cudaMalloc(&sc->buf.tile_start, (size_t)(n + 1) * 4));

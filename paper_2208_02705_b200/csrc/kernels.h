@@ -37,7 +37,10 @@ struct ChunkBuffers {
   uint32_t* ray_cnt;     // [n_rays] segments per ray
   uint32_t* ray_off;     // [n_rays] block-local exclusive offset after count; global after emit
   uint32_t* block_sum;   // [n_blocks] segments per sampler block -> exclusive scan in place
-  uint32_t* bin_cnt;     // [n] segments per subfield
+  uint32_t* bin_cnt;     // [n] segments per subfield reserved by sampler blocks (k_count); total after k_scan
+  uint32_t* bin_ovf;     // [n] segments per subfield that no block reserved (a block's list was full)
+  uint2* blk_list;       // [n_blocks][kBlkListCap] (subfield, first position inside its bin) reserved by the block
+  uint32_t* blk_list_n;  // [n_blocks] entries used
   uint32_t* bin_start;   // [n+1]
   uint32_t* bin_cursor;  // [n]
   uint32_t* tile_start;  // [n+1] first MLP tile of each subfield
@@ -55,13 +58,14 @@ struct ChunkBuffers {
 };
 
 constexpr int kSamplerThreads = 256;
-constexpr int kHitCap = 16;
+constexpr int kHitCap = 64;
+constexpr int kBlkListCap = 256;
 
 void launch_count(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
                   int n_bins, cudaStream_t s);
 void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_tile, cudaStream_t s);
 void launch_emit(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
-                 cudaStream_t s);
+                 int n_bins, cudaStream_t s);
 // fp32 MLP on the FP32 ALUs.  weights_t: per subfield, per layer W^T[in][out] then b[out].
 cudaError_t launch_mlp_fp32(const GridParams& g, const FrameParams& f, const ChunkBuffers& b,
                             const NetShape& net, const Fp32Layout& lay, const float* weights_t,

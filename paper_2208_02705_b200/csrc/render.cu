@@ -99,7 +99,10 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
     sc->buf.dirblk = nullptr;
   }
   cudaStream_t s = sc->stream;
+  if ((st = grow(sc->buf.blk_list, sc->blk_list_cap, n_blocks * kBlkListCap, 1, 1)) != R360_OK) return st;
+  if ((st = grow(sc->buf.blk_list_n, sc->blk_list_n_cap, n_blocks, 1, 1)) != R360_OK) return st;
   R360_CUDA(cudaMemsetAsync(sc->buf.bin_cnt, 0, (size_t)n * 4, s));
+  R360_CUDA(cudaMemsetAsync(sc->buf.bin_ovf, 0, (size_t)n * 4, s));
   if (ev) cudaEventRecord(ev->e[0], s);
   launch_count(sc->grid_p, sc->d_grid, f, sc->buf, n, s);
   if (ev) cudaEventRecord(ev->e[1], s);
@@ -121,7 +124,7 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
       if ((st = grow(sc->d_rec_dir, sc->rec_dir_cap, n_segs)) != R360_OK) return st;
       sc->buf.rec_dir = sc->d_rec_dir;
     }
-    launch_emit(sc->grid_p, sc->d_grid, f, sc->buf, s);
+    launch_emit(sc->grid_p, sc->d_grid, f, sc->buf, n, s);
     launches += 1;
     R360_CUDA(cudaGetLastError());
   }

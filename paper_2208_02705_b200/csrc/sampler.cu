@@ -83,7 +83,7 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
       if ((peers & lanemask_lt()) == 0) {
         uint32_t c = __popc(peers);
         if (use_smem_hist) atomicAdd(&hist[lab], c);
-        else atomicAdd(&b.bin_cnt[lab], c);
+        else atomicAdd(&b.bin_ovf[lab], c);
       }
     }
   }
@@ -95,11 +95,25 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
   }
   if (threadIdx.x == 0) b.block_sum[blockIdx.x] = total;
   if (use_smem_hist) {
+    // The block RESERVES its share of every bin it touched: one returning atomic per (block, subfield),
+    // remembered in the block's list, so that k_emit places this block's segments with shared-memory
+    // cursors and no global atomics (thousands of warps hit the same few subfields at the same time).
+    __shared__ uint32_t list_n;
+    if (threadIdx.x == 0) list_n = 0;
     __syncthreads();
+    uint2* list = b.blk_list + (size_t)blockIdx.x * kBlkListCap;
     for (int k = threadIdx.x; k < n_bins; k += blockDim.x) {
-      uint32_t c = hist[k];
-      if (c) atomicAdd(&b.bin_cnt[k], c);
+      const uint32_t c = hist[k];
+      if (c) {
+        const uint32_t i = atomicAdd(&list_n, 1u);
+        if (i < (uint32_t)kBlkListCap) list[i] = make_uint2((uint32_t)k, atomicAdd(&b.bin_cnt[k], c));
+        else atomicAdd(&b.bin_ovf[k], c);          // list full: k_emit falls back to the global cursor
+      }
     }
+    __syncthreads();
+    if (threadIdx.x == 0) b.blk_list_n[blockIdx.x] = min(list_n, (uint32_t)kBlkListCap);
+  } else if (threadIdx.x == 0) {
+    b.blk_list_n[blockIdx.x] = 0;
   }
 }
 
@@ -150,6 +164,13 @@ k_scan(ChunkBuffers b, int n_blocks, int n_bins, int segs_per_tile) {
     uint64_t tot = scan_array(b.block_sum, b.block_sum, n_blocks, sm, 0, nullptr);
     if (threadIdx.x == 0) b.totals[0] = tot;
   } else {
+    // a bin = [segments reserved by blocks | the rest, placed through the global cursor]
+    for (int k = threadIdx.x; k < n_bins; k += blockDim.x) {
+      const uint32_t res = b.bin_cnt[k];
+      b.bin_cursor[k] = res;
+      b.bin_cnt[k] = res + b.bin_ovf[k];
+    }
+    __syncthreads();
     // tile counts first (they read bin_cnt), then the bin starts
     uint64_t tiles = scan_array(nullptr, b.tile_start, n_bins, sm, segs_per_tile, b.bin_cnt);
     uint64_t segs = scan_array(b.bin_cnt, b.bin_start, n_bins, sm, 0, nullptr);
@@ -158,13 +179,26 @@ k_scan(ChunkBuffers b, int n_blocks, int n_bins, int segs_per_tile) {
       b.bin_start[n_bins] = (uint32_t)segs;
       b.totals[1] = tiles;
     }
-    for (int k = threadIdx.x; k < n_bins; k += blockDim.x) b.bin_cursor[k] = 0;
   }
 }
 
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kSamplerThreads)
-k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuffers b) {
+k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuffers b, int n_bins,
+       int use_smem_cursor) {
+  extern __shared__ uint32_t cur[];      // [n_bins] when use_smem_cursor: next position of this block in each bin
+  constexpr uint32_t kNotReserved = 0xFFFFFFFFu;
+  if (use_smem_cursor) {
+    for (int k = threadIdx.x; k < n_bins; k += blockDim.x) cur[k] = kNotReserved;
+    __syncthreads();
+    const uint2* list = b.blk_list + (size_t)blockIdx.x * kBlkListCap;
+    const uint32_t n = b.blk_list_n[blockIdx.x];
+    for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+      const uint2 e = list[i];
+      cur[e.x] = __ldg(b.bin_start + e.x) + e.y;
+    }
+    __syncthreads();
+  }
   const unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = r < f.n_rays;
   Walker w;
@@ -207,9 +241,13 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
       unsigned peers = __match_any_sync(m, lab);
       int leader = __ffs(peers) - 1;
       uint32_t base = 0;
-      if ((int)(threadIdx.x & 31) == leader) base = atomicAdd(&b.bin_cursor[lab], (uint32_t)__popc(peers));
+      if ((int)(threadIdx.x & 31) == leader) {
+        const uint32_t c = (uint32_t)__popc(peers);
+        if (use_smem_cursor && cur[lab] != kNotReserved) base = atomicAdd(&cur[lab], c);   // reserved by k_count
+        else base = __ldg(b.bin_start + lab) + atomicAdd(&b.bin_cursor[lab], c);
+      }
       base = __shfl_sync(peers, base, leader);
-      uint32_t pos = __ldg(b.bin_start + lab) + base + __popc(peers & lanemask_lt());
+      uint32_t pos = base + __popc(peers & lanemask_lt());
       b.recs[pos] = make_uint4(r, __float_as_uint(t_in), __float_as_uint(dt), slot);
       if (b.rec_dir) b.rec_dir[pos] = dir;
       b.seg_tin[slot] = t_in;
@@ -261,9 +299,11 @@ void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_t
 }
 
 void launch_emit(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
-                 cudaStream_t s) {
+                 int n_bins, cudaStream_t s) {
   int blocks = (f.n_rays + kSamplerThreads - 1) / kSamplerThreads;
-  k_emit<<<blocks, kSamplerThreads, 0, s>>>(g, grid, f, b);
+  int use_smem = n_bins <= 8192;
+  size_t smem = use_smem ? (size_t)n_bins * sizeof(uint32_t) : 0;
+  k_emit<<<blocks, kSamplerThreads, smem, s>>>(g, grid, f, b, n_bins, use_smem);
 }
 
 void launch_export_samples(const GridParams& g, const ChunkBuffers& b, int n_bins, unsigned n_segs,
