@@ -75,6 +75,10 @@ class Oracle:
         L.r360o_samples_rows.restype = C.c_int64
         L.r360o_samples_rows.argtypes = [C.c_void_p, _PF, _I, _I, _I, _I, _PU, C.c_int64, _PF, _PI]
         L.r360o_num_threads.restype = C.c_int
+        L.r360o_ray_pinhole.argtypes = [_PF, _D, _D, _D, _D, _I, _I, _PF, _PF]
+        L.r360o_pinhole_tables.argtypes = [_I, _I, _D, _D, _D, _D, _PF, _PF]
+        L.r360o_set_camera.restype = C.c_int
+        L.r360o_set_camera.argtypes = [C.c_void_p, _I, _D, _D, _D, _D]
 
     # ---- scene-independent taps
     def num_threads(self):
@@ -100,6 +104,12 @@ class Oracle:
         pose = np.ascontiguousarray(pose, np.float32).reshape(12)
         o, d = np.empty(3, np.float32), np.empty(3, np.float32)
         self.lib.r360o_ray(_p(pose, _F), W, H, i, j, _p(o, _F), _p(d, _F))
+        return o, d
+
+    def ray_pinhole(self, pose, fx, fy, cx, cy, i, j):
+        pose = np.ascontiguousarray(pose, np.float32).reshape(12)
+        o, d = np.empty(3, np.float32), np.empty(3, np.float32)
+        self.lib.r360o_ray_pinhole(_p(pose, _F), fx, fy, cx, cy, i, j, _p(o, _F), _p(d, _F))
         return o, d
 
     def pe(self, x, L):
@@ -164,6 +174,12 @@ class OracleScene:
         if self.h:
             self.o.lib.r360o_destroy(self.h)
             self.h = None
+
+    def set_camera(self, model="equirect", fx=0.0, fy=0.0, cx=0.0, cy=0.0):
+        """Camera of the following ray_samples / samples_rows / render_* calls (reading P for "pinhole")."""
+        m = {"equirect": 0, "pinhole": 1}[model]
+        if self.o.lib.r360o_set_camera(self.h, m, fx, fy, cx, cy) != 0:
+            raise ValueError("r360o_set_camera rejected the camera")
 
     def __del__(self):
         try:

@@ -25,6 +25,8 @@ struct r360o_scene {
   float* w;             /* n*P */
   float* centre;        /* n*3 (A3) */
   float* inv_half;      /* n*3 (A3) */
+  int32_t cam_model;    /* 0 = equirectangular (Eq.2-3), 1 = pinhole (reading P) */
+  double fx, fy, cx, cy;
 };
 
 /* ---------------------------------------------------------------- layout (A1)
@@ -179,6 +181,67 @@ void r360o_ray(const float pose[12], int32_t W, int32_t H, int32_t i, int32_t j,
   o[0] = pose[3]; o[1] = pose[7]; o[2] = pose[11];
 }
 
+/* ---------------------------------------------------------------- pinhole view (reading P)
+ * The paper shows "perspective views" while roaming (720p timings :200) and gives no
+ * camera model.  Reading P: the standard pinhole in the camera frame of Eq.3 (x right, y down, z
+ * forward): pixel centre (i+0.5, j+0.5) -> x = (i + 0.5 - cx)/fx, y = (j + 0.5 - cy)/fy,
+ * binary64, rounded once to binary32 (tables, like B2); d_cam = (x, y, 1)/|(x, y, 1)| in binary32,
+ * every operation rounded: n2 = (x*x + y*y) + 1, inv = 1/sqrt(n2), d_cam = (x*inv, y*inv, inv);
+ * then d = R d_cam as in B3.  t stays the metric distance along the unit ray (as for the panorama). */
+void r360o_pinhole_tables(int32_t W, int32_t H, double fx, double fy, double cx, double cy, float* x, float* y) {
+  for (int32_t i = 0; i < W; ++i) x[i] = (float)((((double)i + 0.5) - cx) / fx);
+  for (int32_t j = 0; j < H; ++j) y[j] = (float)((((double)j + 0.5) - cy) / fy);
+}
+
+static void pinhole_dir(const float pose[12], float x, float y, float d[3]) {
+  float xx = x * x;
+  float yy = y * y;
+  float s2 = xx + yy;
+  float n2 = s2 + 1.0f;
+  float inv = 1.0f / sqrtf(n2);
+  float c[3];
+  c[0] = x * inv;
+  c[1] = y * inv;
+  c[2] = inv;
+  for (int a = 0; a < 3; ++a) {
+    float m0 = pose[a * 4 + 0] * c[0];
+    float m1 = pose[a * 4 + 1] * c[1];
+    float m2 = pose[a * 4 + 2] * c[2];
+    float s01 = m0 + m1;
+    d[a] = s01 + m2;
+  }
+}
+
+void r360o_ray_pinhole(const float pose[12], double fx, double fy, double cx, double cy, int32_t i, int32_t j,
+                       float o[3], float d[3]) {
+  float x = (float)((((double)i + 0.5) - cx) / fx);
+  float y = (float)((((double)j + 0.5) - cy) / fy);
+  pinhole_dir(pose, x, y, d);
+  o[0] = pose[3]; o[1] = pose[7]; o[2] = pose[11];
+}
+
+int r360o_set_camera(r360o_scene* s, int32_t model, double fx, double fy, double cx, double cy) {
+  if (!s || (model != 0 && model != 1)) return 1;
+  if (model == 1 && !(fx > 0.0 && fy > 0.0 && isfinite(fx) && isfinite(fy) && isfinite(cx) && isfinite(cy))) return 1;
+  s->cam_model = model; s->fx = fx; s->fy = fy; s->cx = cx; s->cy = cy;
+  return 0;
+}
+
+/* per-image tables of the scene's camera: 2W + 2H floats (equirect: sin/cos phi, sin/cos theta;
+ * pinhole: x in the first W, y in the third block, the rest unused) and the direction of pixel (i,j) */
+static float* camera_tables(const r360o_scene* s, int32_t W, int32_t H) {
+  float* tab = (float*)calloc((size_t)(2 * W + 2 * H), sizeof(float));
+  if (s->cam_model == 1) r360o_pinhole_tables(W, H, s->fx, s->fy, s->cx, s->cy, tab, tab + 2 * W);
+  else r360o_trig_tables(W, H, tab, tab + W, tab + 2 * W, tab + 2 * W + H);
+  return tab;
+}
+
+static void camera_dir(const r360o_scene* s, const float pose[12], const float* tab, int32_t W, int32_t H,
+                       int i, int j, float d[3]) {
+  if (s->cam_model == 1) pinhole_dir(pose, tab[i], tab[2 * W + j], d);
+  else ray_dir(pose, tab[i], tab[W + i], tab[2 * W + j], tab[2 * W + H + j], d);
+}
+
 /* ---------------------------------------------------------------- traversal (C)
  * PAPER.md:174 "ray casting techniques to quickly localize occupied voxels";
  * :29 / :105 empty-space skipping. */
@@ -331,7 +394,8 @@ static int64_t ray_samples(const r360o_scene* s, const float o[3], const float d
 int64_t r360o_ray_samples(const r360o_scene* s, const float pose[12], int32_t W, int32_t H,
                           int32_t i, int32_t j, int64_t cap, float* t, float* delta, int32_t* subfield) {
   float o[3], d[3];
-  r360o_ray(pose, W, H, i, j, o, d);
+  if (s->cam_model == 1) r360o_ray_pinhole(pose, s->fx, s->fy, s->cx, s->cy, i, j, o, d);
+  else r360o_ray(pose, W, H, i, j, o, d);
   return ray_samples(s, o, d, cap, t, delta, subfield);
 }
 
@@ -484,12 +548,12 @@ static void render_visit(void* vctx, int64_t v, float t_in, float t_out, int occ
   }
 }
 
-static void render_pixel(const r360o_scene* s, const float pose[12], const float* sp, const float* cp,
-                         const float* st, const float* ct, int i, int j, int64_t slot,
+static void render_pixel(const r360o_scene* s, const float pose[12], const float* tab, int32_t W, int32_t H,
+                         int i, int j, int64_t slot,
                          float* rgb, float* depth, float* rgb_full, float* depth_full,
                          float* ambiguity, uint32_t* n_emitted, uint32_t* n_used) {
   float o[3] = {pose[3], pose[7], pose[11]}, d[3];
-  ray_dir(pose, sp[i], cp[i], st[j], ct[j], d);
+  camera_dir(s, pose, tab, W, H, i, j, d);
   ray_t r;
   ray_setup(&r, o, d);
   render_t c;
@@ -516,15 +580,13 @@ int r360o_render_pixels(const r360o_scene* s, const float pose[12], int32_t W, i
                         float* ambiguity, uint32_t* n_emitted, uint32_t* n_used) {
   if (!s || !pose || W < 1 || H < 1 || n_pix < 0) return 1;
   for (int a = 0; a < 12; ++a) if (!isfinite(pose[a])) return 1;
-  float* tab = (float*)malloc((size_t)(2 * W + 2 * H) * sizeof(float));
-  float *sp = tab, *cp = tab + W, *st = tab + 2 * W, *ct = tab + 2 * W + H;
-  r360o_trig_tables(W, H, sp, cp, st, ct);
+  float* tab = camera_tables(s, W, H);
   int bad = 0;
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t q = 0; q < n_pix; ++q) {
     int i = px[q], j = py[q];
     if (i < 0 || i >= W || j < 0 || j >= H) { bad = 1; continue; }
-    render_pixel(s, pose, sp, cp, st, ct, i, j, q, rgb, depth, rgb_full, depth_full, ambiguity, n_emitted, n_used);
+    render_pixel(s, pose, tab, W, H, i, j, q, rgb, depth, rgb_full, depth_full, ambiguity, n_emitted, n_used);
   }
   free(tab);
   return bad;
@@ -536,14 +598,12 @@ int r360o_render_rows(const r360o_scene* s, const float pose[12], int32_t W, int
                       float* ambiguity, uint32_t* n_emitted, uint32_t* n_used) {
   if (!s || !pose || W < 1 || H < 1 || row0 < 0 || row1 > H || row0 > row1) return 1;
   for (int a = 0; a < 12; ++a) if (!isfinite(pose[a])) return 1;
-  float* tab = (float*)malloc((size_t)(2 * W + 2 * H) * sizeof(float));
-  float *sp = tab, *cp = tab + W, *st = tab + 2 * W, *ct = tab + 2 * W + H;
-  r360o_trig_tables(W, H, sp, cp, st, ct);
+  float* tab = camera_tables(s, W, H);
   int64_t n_pix = (int64_t)(row1 - row0) * W;
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t q = 0; q < n_pix; ++q) {
     int i = (int)(q % W), j = row0 + (int)(q / W);
-    render_pixel(s, pose, sp, cp, st, ct, i, j, q, rgb, depth, rgb_full, depth_full, ambiguity, n_emitted, n_used);
+    render_pixel(s, pose, tab, W, H, i, j, q, rgb, depth, rgb_full, depth_full, ambiguity, n_emitted, n_used);
   }
   free(tab);
   return 0;
@@ -556,14 +616,12 @@ int64_t r360o_samples_rows(const r360o_scene* s, const float pose[12], int32_t W
                            int32_t row0, int32_t row1, uint32_t* counts, int64_t cap, float* t,
                            int32_t* subfield) {
   int64_t n_pix = (int64_t)(row1 - row0) * W;
-  float* tab = (float*)malloc((size_t)(2 * W + 2 * H) * sizeof(float));
-  float *sp = tab, *cp = tab + W, *st = tab + 2 * W, *ct = tab + 2 * W + H;
-  r360o_trig_tables(W, H, sp, cp, st, ct);
+  float* tab = camera_tables(s, W, H);
   float o[3] = {pose[3], pose[7], pose[11]};
 #pragma omp parallel for schedule(dynamic, 64)
   for (int64_t q = 0; q < n_pix; ++q) {
     float d[3];
-    ray_dir(pose, sp[q % W], cp[q % W], st[row0 + q / W], ct[row0 + q / W], d);
+    camera_dir(s, pose, tab, W, H, (int)(q % W), row0 + (int)(q / W), d);
     counts[q] = (uint32_t)ray_samples(s, o, d, 0, NULL, NULL, NULL);
   }
   int64_t total = 0;
@@ -577,7 +635,7 @@ int64_t r360o_samples_rows(const r360o_scene* s, const float pose[12], int32_t W
 #pragma omp parallel for schedule(dynamic, 64)
     for (int64_t q = 0; q < n_pix; ++q) {
       float d[3];
-      ray_dir(pose, sp[q % W], cp[q % W], st[row0 + q / W], ct[row0 + q / W], d);
+      camera_dir(s, pose, tab, W, H, (int)(q % W), row0 + (int)(q / W), d);
       ray_samples(s, o, d, counts[q], t + off[q], dl + off[q], subfield + off[q]);
     }
     free(dl);

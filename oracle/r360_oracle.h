@@ -65,6 +65,16 @@ void r360o_pixel_to_sphere(int32_t i, int32_t j, int32_t W, int32_t H, double* p
 /* Ray of pixel (i,j): o = pose translation, d = R * Eq.3 direction (binary32, B3). */
 void r360o_ray(const float pose[12], int32_t W, int32_t H, int32_t i, int32_t j, float o[3], float d[3]);
 
+/* Pinhole view (reading P; the paper's perspective display, gives no model):
+ * x_i = (i + 0.5 - cx)/fx, y_j = (j + 0.5 - cy)/fy in binary64 rounded once to binary32;
+ * d_cam = (x, y, 1)/|(x, y, 1)| in binary32 (n2 = (x*x + y*y) + 1, inv = 1/sqrt(n2)); d = R d_cam (B3). */
+void r360o_pinhole_tables(int32_t W, int32_t H, double fx, double fy, double cx, double cy, float* x, float* y);
+void r360o_ray_pinhole(const float pose[12], double fx, double fy, double cx, double cy, int32_t i, int32_t j,
+                       float o[3], float d[3]);
+/* Camera used by r360o_ray_samples / render_* / samples_rows of this scene: model 0 = equirectangular
+ * (default), 1 = pinhole with the given intrinsics (pixels).  Returns 0 on success. */
+int r360o_set_camera(r360o_scene* s, int32_t model, double fx, double fy, double cx, double cy);
+
 /* Voxel walk (readings C1-C5).  Writes up to cap crossed voxels front to back;
  * only_occupied != 0 keeps occupied voxels only.  Returns the number found
  * (may exceed cap; then only cap were written). */
