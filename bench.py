@@ -162,8 +162,9 @@ def workload_config(sc, args, precision):
             "l2": "explicit L2 flush (512 MiB memset) between timed iterations, outside the CUDA events"}
 
 
-def time_config(r360, config, precision, steps=5, warmup=3):
-    """Short device-timed run of another BASELINE.json config (all its poses in one batch call)."""
+def time_config(r360, config, precision, steps=5, warmup=3, pinhole=None):
+    """Short device-timed run of another BASELINE.json config (all its poses in one batch call).
+    pinhole = (W, H, f): the same scene through the roaming (perspective) view instead of the panorama."""
     import torch
     from scenegen import make_scene
     sc = make_scene(config)
@@ -171,6 +172,9 @@ def time_config(r360, config, precision, steps=5, warmup=3):
     scene.set_precision(precision)
     scene.use_current_torch_stream()
     B, W, H = len(sc.poses), sc.W, sc.H
+    if pinhole:
+        W, H, f = pinhole
+        scene.set_camera("pinhole", f, f, W / 2.0, H / 2.0)
     poses = np.ascontiguousarray(np.stack([np.asarray(p, np.float32) for p in sc.poses]))
     rgb = torch.empty((B, H, W, 3), dtype=torch.float32, device="cuda")
     depth = torch.empty((B, H, W), dtype=torch.float32, device="cuda")
@@ -192,7 +196,7 @@ def time_config(r360, config, precision, steps=5, warmup=3):
     ms_mlp /= steps
     fl = flop_per_sample(sc.hidden_width, sc.n_hidden)
     peaks = measured_peaks()
-    out = {"config": config, "name": sc.name, "image": [W, H], "poses": B, "n_subfields": sc.n_subfields,
+    out = {"config": config, "name": sc.name + (" (pinhole view)" if pinhole else ""), "image": [W, H], "poses": B, "n_subfields": sc.n_subfields,
            "mlp": [sc.n_hidden, sc.hidden_width], "K": sc.samples_per_voxel, "precision": precision,
            "ms_per_step": ms, "rays_per_s": B * W * H / (ms * 1e-3), "fps": B * 1e3 / ms,
            "samples_per_step": int(st.samples_emitted), "mlp_samples_per_s": st.samples_emitted / (ms_mlp * 1e-3),
@@ -339,6 +343,8 @@ def main():
             scene.close()
             del rgb, depth
             line["other_configs"] = [time_config(r360, c, precision) for c in (1, 2, 4, 5) if c != args.config]
+            # the paper times its perspective (roaming) view at 720p: same scene, 90 degree pinhole
+            line["other_configs"].append(time_config(r360, args.config, precision, pinhole=(1280, 720, 640.0)))
         if not args.no_cpu_baseline:
             cb = oracle_sample(sc, args.ref_row_stride)
             line["cpu_baseline"] = {"value": cb["rays_per_s"], "unit": "rays/s", "cores": cb["cores"],

@@ -96,6 +96,15 @@ r360_status r360_render_batch(r360_scene* scene, const float* poses, int32_t B, 
 r360_status r360_render_batch_host(r360_scene* scene, const float* poses, int32_t B, int32_t W, int32_t H,
                                    float* out_rgb_host, float* out_depth_host);
 
+/* Camera of the following render / debug calls.  model 0 (default) = the equirectangular panorama of
+ * Eq.2-3; model 1 = pinhole view for roaming (the paper's perspective display,
+ * PAPER.md:206, :200, gives no model; reading P): pixel centre (i+0.5, j+0.5) ->
+ * x = (i + 0.5 - cx)/fx, y = (j + 0.5 - cy)/fy (binary64, rounded once to binary32),
+ * d_cam = (x, y, 1)/|(x, y, 1)| in the camera frame of Eq.3 (x right, y down, z forward), d = R d_cam;
+ * depth stays the distance along the unit ray.  fx, fy, cx, cy in pixels; fx, fy > 0; ignored for model 0.
+ * Returns R360_ERR_INVALID_ARG for another model or non-finite / non-positive intrinsics. */
+r360_status r360_set_camera(r360_scene* scene, int32_t model, double fx, double fy, double cx, double cy);
+
 /* 0 = fp32 MLP on the FP32 ALUs (default); 1 = bf16 tensor-core MLP (tcgen05, fp32 accumulate). */
 r360_status r360_set_precision(r360_scene* scene, int32_t mode);
 /* CUDA stream (cudaStream_t / CUstream as void*) all work of this scene is enqueued on. */

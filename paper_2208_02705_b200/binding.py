@@ -67,6 +67,8 @@ def lib():
     L.r360_render_batch_host.argtypes = [vp, f32p, i32, i32, i32, vp, vp]
     L.r360_set_precision.restype = C.c_int
     L.r360_set_precision.argtypes = [vp, i32]
+    L.r360_set_camera.restype = C.c_int
+    L.r360_set_camera.argtypes = [vp, i32, C.c_double, C.c_double, C.c_double, C.c_double]
     L.r360_set_stream.restype = C.c_int
     L.r360_set_stream.argtypes = [vp, vp]
     L.r360_set_chunk_rays.restype = C.c_int
@@ -153,6 +155,10 @@ class Scene:
 
     def set_precision(self, mode):
         _check(lib().r360_set_precision(self._h, {"fp32": 0, "bf16": 1}.get(mode, mode)), "r360_set_precision")
+
+    def set_camera(self, model="equirect", fx=0.0, fy=0.0, cx=0.0, cy=0.0):
+        _check(lib().r360_set_camera(self._h, {"equirect": 0, "pinhole": 1}.get(model, model), fx, fy, cx, cy),
+               "r360_set_camera")
 
     def set_stream(self, cuda_stream_ptr):
         _check(lib().r360_set_stream(self._h, C.c_void_p(cuda_stream_ptr)), "r360_set_stream")

@@ -33,10 +33,11 @@ struct FrameParams {
   unsigned pose0;        // ray0 / (W*H)
   unsigned pix0;         // ray0 % (W*H)
   unsigned n_rays;       // rays in this chunk
+  int camera;            // 0 equirect (Eq.2-3), 1 pinhole (reading P)
   const float* poses;    // device [B*12]
-  const float* sin_phi;  // device [W]  (reading B2: host binary64 libm, rounded once)
+  const float* sin_phi;  // device [W]  (reading B2: host binary64 libm, rounded once); pinhole: x_i
   const float* cos_phi;
-  const float* sin_theta;  // device [H]
+  const float* sin_theta;  // device [H]; pinhole: y_j
   const float* cos_theta;
 };
 
@@ -62,11 +63,22 @@ __device__ __forceinline__ Ray make_ray(const FrameParams& f, unsigned r) {
   const unsigned j = pix / (unsigned)f.W;
   const unsigned i = pix - j * (unsigned)f.W;
   const float* P = f.poses + b * 12;
-  float sp = __ldg(f.sin_phi + i), cp = __ldg(f.cos_phi + i);
-  float st = __ldg(f.sin_theta + j), ct = __ldg(f.cos_theta + j);
-  float x = __fmul_rn(ct, sp);
-  float y = -st;
-  float z = __fmul_rn(ct, cp);
+  float x, y, z;
+  if (f.camera == 0) {
+    float sp = __ldg(f.sin_phi + i), cp = __ldg(f.cos_phi + i);
+    float st = __ldg(f.sin_theta + j), ct = __ldg(f.cos_theta + j);
+    x = __fmul_rn(ct, sp);
+    y = -st;
+    z = __fmul_rn(ct, cp);
+  } else {
+    // reading P: d_cam = (x, y, 1)/|(x, y, 1)|, n2 = (x*x + y*y) + 1, inv = 1/sqrt(n2), each operation rounded
+    const float px = __ldg(f.sin_phi + i), py = __ldg(f.sin_theta + j);
+    const float n2 = __fadd_rn(__fadd_rn(__fmul_rn(px, px), __fmul_rn(py, py)), 1.0f);
+    const float inv = __fdiv_rn(1.0f, __fsqrt_rn(n2));
+    x = __fmul_rn(px, inv);
+    y = __fmul_rn(py, inv);
+    z = inv;
+  }
   Ray ray;
   ray.pose = b;
 #pragma unroll

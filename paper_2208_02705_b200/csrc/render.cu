@@ -23,14 +23,21 @@ r360_status grow(T*& p, size_t& cap, size_t need, size_t slack_num = 5, size_t s
 
 // Reading B1/B2: pixel-centre angles and their trig in binary64 libm, rounded once to binary32.
 r360_status ensure_tables(r360_scene* sc, int W, int H) {
-  if (sc->d_tables && sc->tab_W == W && sc->tab_H == H) return R360_OK;
-  std::vector<float> t((size_t)2 * W + 2 * H);
-  for (int i = 0; i < W; ++i) {
+  if (sc->d_tables && sc->tab_W == W && sc->tab_H == H && sc->tab_cam_model == sc->cam_model &&
+      (sc->cam_model == 0 || std::memcmp(sc->tab_cam, sc->cam, sizeof(sc->cam)) == 0))
+    return R360_OK;
+  std::vector<float> t((size_t)2 * W + 2 * H, 0.0f);
+  if (sc->cam_model == 1) {
+    // reading P: x_i = (i + 0.5 - cx)/fx, y_j = (j + 0.5 - cy)/fy in binary64, rounded once to binary32
+    for (int i = 0; i < W; ++i) t[i] = (float)((((double)i + 0.5) - sc->cam[2]) / sc->cam[0]);
+    for (int j = 0; j < H; ++j) t[(size_t)2 * W + j] = (float)((((double)j + 0.5) - sc->cam[3]) / sc->cam[1]);
+  }
+  for (int i = 0; i < W && sc->cam_model == 0; ++i) {
     double phi = (((double)i + 0.5) - (double)W / 2.0) * (2.0 * kPi / (double)W);
     t[i] = (float)std::sin(phi);
     t[(size_t)W + i] = (float)std::cos(phi);
   }
-  for (int j = 0; j < H; ++j) {
+  for (int j = 0; j < H && sc->cam_model == 0; ++j) {
     double theta = -((((double)j + 0.5) - (double)H / 2.0) * (kPi / (double)H));
     t[(size_t)2 * W + j] = (float)std::sin(theta);
     t[(size_t)2 * W + H + j] = (float)std::cos(theta);
@@ -42,6 +49,8 @@ r360_status ensure_tables(r360_scene* sc, int W, int H) {
   R360_CUDA(cudaStreamSynchronize(sc->stream));
   sc->tab_W = W;
   sc->tab_H = H;
+  sc->tab_cam_model = sc->cam_model;
+  std::memcpy(sc->tab_cam, sc->cam, sizeof(sc->cam));
   return R360_OK;
 }
 
@@ -63,6 +72,7 @@ FrameParams frame_params(const r360_scene* sc, int W, int H, long long ray0, uns
   f.W = W; f.H = H; f.ray0 = ray0; f.n_rays = n_rays;
   f.pose0 = (unsigned)(ray0 / ((long long)W * H));
   f.pix0 = (unsigned)(ray0 % ((long long)W * H));
+  f.camera = sc->cam_model;
   f.poses = sc->d_poses;
   f.sin_phi = sc->d_tables;
   f.cos_phi = sc->d_tables + W;
@@ -220,6 +230,16 @@ r360_status r360_set_precision(r360_scene* sc, int32_t mode) {
   if (!sc || (mode != 0 && mode != 1)) return R360_ERR_INVALID_ARG;
   if (mode == 1 && !sc->d_wpack) return R360_ERR_INVALID_ARG;
   sc->precision = mode;
+  return R360_OK;
+}
+
+r360_status r360_set_camera(r360_scene* sc, int32_t model, double fx, double fy, double cx, double cy) {
+  if (!sc || (model != 0 && model != 1)) return R360_ERR_INVALID_ARG;
+  if (model == 1 && !(fx > 0.0 && fy > 0.0 && std::isfinite(fx) && std::isfinite(fy) && std::isfinite(cx) &&
+                      std::isfinite(cy)))
+    return R360_ERR_INVALID_ARG;
+  sc->cam_model = model;
+  sc->cam[0] = fx; sc->cam[1] = fy; sc->cam[2] = cx; sc->cam[3] = cy;
   return R360_OK;
 }
 

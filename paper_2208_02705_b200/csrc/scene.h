@@ -21,6 +21,11 @@ struct r360_scene {
   // per (W,H): trig tables; per call: poses
   float* d_tables = nullptr;
   int tab_W = 0, tab_H = 0;
+  // camera (r360_set_camera): 0 equirect, 1 pinhole; tab_cam = what d_tables was built for
+  int cam_model = 0;
+  double cam[4] = {0, 0, 0, 0};             // fx, fy, cx, cy
+  int tab_cam_model = -1;
+  double tab_cam[4] = {0, 0, 0, 0};
   float* d_poses = nullptr;
   int poses_cap = 0;
   // chunk buffers and capacities

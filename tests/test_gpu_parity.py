@@ -194,3 +194,39 @@ def test_full_size_config3_sampled(r360, oracle):
         idx = np.repeat(offsets[row].astype(np.int64), oc64) + (np.arange(int(oc64.sum())) - np.repeat(np.cumsum(oc64) - oc64, oc64))
         assert np.array_equal(t_np[idx], ot.view(np.uint32))
         assert np.array_equal(sid_np[idx], osid)
+
+
+@pytest.mark.parametrize("config,W,H,f", [(1, 160, 90, 80.0), (2, 320, 180, 200.0), (1, 37, 19, 11.5)])
+def test_pinhole_view(r360, oracle, config, W, H, f):
+    """The roaming (perspective) view, reading P: samples bit-exact, fp32 image within 1e-4, bf16 within 2e-3."""
+    sc = get_scene(config)
+    cam = ("pinhole", f, f * 1.1, W / 2.0 + 0.25, H / 2.0 - 0.5)
+    ora = oracle.scene_from(sc)
+    ora.set_camera(*cam)
+    gpu = r360.scene_from(sc)
+    gpu.set_camera(*cam)
+    pose = sc.poses[0]
+    counts, offsets, t, sid = gpu.debug_samples(pose, W, H)
+    oc, ot, osid = ora.samples_rows(pose, W, H)
+    counts, offsets = counts.cpu().numpy().view(np.uint32), offsets.cpu().numpy().view(np.uint32)
+    assert np.array_equal(counts, oc)
+    idx = ray_major_index(counts, offsets)
+    assert np.array_equal(t.cpu().numpy().view(np.uint32)[idx], ot.view(np.uint32))
+    assert np.array_equal(sid.cpu().numpy()[idx], osid)
+    ref = ora.render_rows(pose, W, H)
+    rgb, depth = gpu.render(pose, W, H)
+    check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 1e-4)
+    gpu.set_precision("bf16")
+    rgb, depth = gpu.render(pose, W, H)
+    t_max = float(np.linalg.norm(np.array(sc.box_max) - np.array(sc.box_min)))
+    check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 2e-3, amb_band=0.2, depth_tol=2e-3 * t_max)
+    # back to the panorama: the tables are rebuilt for the other camera
+    gpu.set_camera("equirect")
+    gpu.set_precision("fp32")
+    ora.set_camera("equirect")
+    rgb, depth = gpu.render(pose, 64, 32)
+    check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ora.render_rows(pose, 64, 32), 1e-4)
+    with pytest.raises(r360.R360Error):
+        gpu.set_camera("pinhole", -1.0, 1.0, 0.0, 0.0)
+    gpu.close()
+    ora.close()
