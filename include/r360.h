@@ -96,6 +96,19 @@ r360_status r360_render_batch(r360_scene* scene, const float* poses, int32_t B, 
 r360_status r360_render_batch_host(r360_scene* scene, const float* poses, int32_t B, int32_t W, int32_t H,
                                    float* out_rgb_host, float* out_depth_host);
 
+/* Algorithm 1, stage II (text :157): geometry-aware assignment of the occupied voxels to
+ * n tiny networks -- "pop an unassigned voxel with the minimum coordinate as the anchor; search s-1 nearest
+ * unassigned neighbours; assign these s voxels to the k-th network", s = S/n.  Readings (S1-S4): the
+ * first S mod n networks take one voxel more; minimum coordinate = smallest linear index; nearest = squared
+ * distance of voxel centres in metres (binary32, each operation rounded); ties to the smaller linear index.
+ * Runs on the current CUDA device.  dims/box as in r360_scene_desc; occupancy: HOST uint8[N], occupied iff
+ * >= occ_threshold (>= 1); labels_out: HOST int32[N], receives the network of every occupied voxel and -1 for
+ * empty ones -- the voxel_subfield input of r360_scene_create.  Caller owns both arrays.
+ * R360_ERR_INVALID_ARG: null pointers, bad dims/box, n < 1, n > S, dims > 65535, S >= 2^25. */
+r360_status r360_assign_subfields(const int32_t dims[3], const float box_min[3], const float box_max[3],
+                                  const uint8_t* occupancy, uint8_t occ_threshold, int32_t n,
+                                  int32_t* labels_out);
+
 /* Camera of the following render / debug calls.  model 0 (default) = the equirectangular panorama of
  * Eq.2-3; model 1 = pinhole view for roaming (the paper's perspective display,
  * PAPER.md:206, :200, gives no model; reading P): pixel centre (i+0.5, j+0.5) ->

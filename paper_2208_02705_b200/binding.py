@@ -67,6 +67,9 @@ def lib():
     L.r360_render_batch_host.argtypes = [vp, f32p, i32, i32, i32, vp, vp]
     L.r360_set_precision.restype = C.c_int
     L.r360_set_precision.argtypes = [vp, i32]
+    L.r360_assign_subfields.restype = C.c_int
+    L.r360_assign_subfields.argtypes = [C.POINTER(C.c_int32), f32p, f32p, C.POINTER(C.c_uint8), C.c_uint8, i32,
+                                        C.POINTER(C.c_int32)]
     L.r360_set_camera.restype = C.c_int
     L.r360_set_camera.argtypes = [vp, i32, C.c_double, C.c_double, C.c_double, C.c_double]
     L.r360_set_stream.restype = C.c_int
@@ -111,6 +114,19 @@ def params_per_subfield(**kw):
     kw.setdefault("dims", (1, 1, 1)); kw.setdefault("box_min", (0, 0, 0)); kw.setdefault("box_max", (1, 1, 1))
     kw.setdefault("n_subfields", 1)
     return int(lib().r360_params_per_subfield(C.byref(make_desc(**kw))))
+
+
+def assign_subfields(occupancy, dims, box_min, box_max, occ_threshold, n):
+    """Algorithm 1 stage II on the GPU (r360_assign_subfields): int32 labels[N], -1 for empty voxels."""
+    occ = np.ascontiguousarray(occupancy, np.uint8).reshape(-1)
+    d = (C.c_int32 * 3)(*[int(v) for v in dims])
+    lo = (C.c_float * 3)(*[float(v) for v in box_min])
+    hi = (C.c_float * 3)(*[float(v) for v in box_max])
+    assert occ.size == d[0] * d[1] * d[2]
+    out = np.empty(occ.size, np.int32)
+    _check(lib().r360_assign_subfields(d, lo, hi, occ.ctypes.data_as(C.POINTER(C.c_uint8)), int(occ_threshold),
+                                       int(n), out.ctypes.data_as(C.POINTER(C.c_int32))), "r360_assign_subfields")
+    return out
 
 
 def _pose_ptr(poses, B):
