@@ -118,6 +118,14 @@ r360_status r360_assign_subfields(const int32_t dims[3], const float box_min[3],
  * Returns R360_ERR_INVALID_ARG for another model or non-finite / non-positive intrinsics. */
 r360_status r360_set_camera(r360_scene* scene, int32_t model, double fx, double fy, double cx, double cy);
 
+/* Wavefronted early termination (0 = off, default; 1 = on).  On: the occupied voxels a ray crosses are fed to
+ * the MLP in passes (crossings [0,2), [2,6), [6,16), [16,64), [64,inf) of every ray); after each pass the compositing step
+ * retires the rays whose transmittance fell below t_threshold (Eq.4-5, reading G), so their remaining samples are
+ * never evaluated.  The images are the same as with 0 (same per-ray sequence of operations); it pays when
+ * surfaces are opaque, as in trained scenes, and costs extra launches when no ray terminates early.  With 1,
+ * r360_stats.segments / mlp_tiles count what reached the MLP, and the per-stage times cover the first pass. */
+r360_status r360_set_wavefront(r360_scene* scene, int32_t enable);
+
 /* 0 = fp32 MLP on the FP32 ALUs (default); 1 = bf16 tensor-core MLP (tcgen05, fp32 accumulate). */
 r360_status r360_set_precision(r360_scene* scene, int32_t mode);
 /* CUDA stream (cudaStream_t / CUstream as void*) all work of this scene is enqueued on. */

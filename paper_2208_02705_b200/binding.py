@@ -70,6 +70,8 @@ def lib():
     L.r360_assign_subfields.restype = C.c_int
     L.r360_assign_subfields.argtypes = [C.POINTER(C.c_int32), f32p, f32p, C.POINTER(C.c_uint8), C.c_uint8, i32,
                                         C.POINTER(C.c_int32)]
+    L.r360_set_wavefront.restype = C.c_int
+    L.r360_set_wavefront.argtypes = [vp, i32]
     L.r360_set_camera.restype = C.c_int
     L.r360_set_camera.argtypes = [vp, i32, C.c_double, C.c_double, C.c_double, C.c_double]
     L.r360_set_stream.restype = C.c_int
@@ -171,6 +173,9 @@ class Scene:
 
     def set_precision(self, mode):
         _check(lib().r360_set_precision(self._h, {"fp32": 0, "bf16": 1}.get(mode, mode)), "r360_set_precision")
+
+    def set_wavefront(self, enable):
+        _check(lib().r360_set_wavefront(self._h, int(bool(enable))), "r360_set_wavefront")
 
     def set_camera(self, model="equirect", fx=0.0, fy=0.0, cx=0.0, cy=0.0):
         _check(lib().r360_set_camera(self._h, {"equirect": 0, "pinhole": 1}.get(model, model), fx, fy, cx, cy),

@@ -161,6 +161,7 @@ void r360_scene_destroy(r360_scene* sc) {
   cudaFree(sc->d_dirblk); cudaFree(sc->d_rec_dir);
   cudaFree(sc->buf.hit_t); cudaFree(sc->buf.hit_lab);
   cudaFree(sc->buf.bin_ovf); cudaFree(sc->buf.blk_list); cudaFree(sc->buf.blk_list_n);
+  cudaFree(sc->d_pass_cnt); cudaFree(sc->buf.pass_off); cudaFree(sc->buf.st_c); cudaFree(sc->buf.st_T);
   cudaFree(sc->d_stage_rgb); cudaFree(sc->d_stage_depth);
   if (sc->h_totals) cudaFreeHost(sc->h_totals);
   for (auto& ce : sc->events)

@@ -8,14 +8,20 @@ namespace r360 {
 
 __global__ void __launch_bounds__(256)
 k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __restrict__ out_rgb,
-            float* __restrict__ out_depth) {
+            float* __restrict__ out_depth, PassParams pp) {
   const unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
   unsigned used = 0;
-  if (r < f.n_rays) {
-    const unsigned cnt = b.ray_cnt[r];
-    const unsigned off = b.ray_off[r];
+  // wavefront pass: rays that finished in an earlier pass have nothing left to do
+  if (r < f.n_rays && !(pp.wavefront && !pp.first && b.st_T[r] < 0.0f)) {
+    const unsigned cnt = pp.wavefront ? b.pass_cnt[r] : b.ray_cnt[r];
+    const unsigned off = pp.wavefront ? b.pass_off[r] : b.ray_off[r];
     const int K = g.K;
     float T = 1.0f, C0 = 0.f, C1 = 0.f, C2 = 0.f, D = 0.f;
+    if (pp.wavefront && !pp.first) {       // the sums continue exactly where the previous pass left them
+      const float4 c = b.st_c[r];
+      C0 = c.x; C1 = c.y; C2 = c.z; D = c.w;
+      T = b.st_T[r];
+    }
     bool done = false;
     for (unsigned s = 0; s < cnt && !done; ++s) {
       const float t_in = b.seg_tin[off + s];
@@ -45,11 +51,25 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __res
         }
       }
     }
-    const size_t gr = (size_t)(f.ray0 + (long long)r);
-    out_rgb[gr * 3 + 0] = C0;
-    out_rgb[gr * 3 + 1] = C1;
-    out_rgb[gr * 3 + 2] = C2;
-    out_depth[gr] = D;
+    bool write_out = true;
+    if (pp.wavefront) {
+      // finished: stopped by tau, no hits beyond this pass, or last pass
+      const bool finished = done || pp.last || b.ray_cnt[r] <= pp.h1;
+      if (!finished) {
+        b.st_c[r] = make_float4(C0, C1, C2, D);
+        b.st_T[r] = T;
+      } else {
+        b.st_T[r] = -1.0f;
+      }
+      write_out = finished;
+    }
+    if (write_out) {
+      const size_t gr = (size_t)(f.ray0 + (long long)r);
+      out_rgb[gr * 3 + 0] = C0;
+      out_rgb[gr * 3 + 1] = C1;
+      out_rgb[gr * 3 + 2] = C2;
+      out_depth[gr] = D;
+    }
   }
   // samples_used statistic
 #pragma unroll
@@ -58,8 +78,8 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __res
 }
 
 void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
-                      float* out_rgb, float* out_depth, cudaStream_t s) {
-  k_composite<<<(f.n_rays + 255) / 256, 256, 0, s>>>(g, f, b, tau, out_rgb, out_depth);
+                      float* out_rgb, float* out_depth, const PassParams& pp, cudaStream_t s) {
+  k_composite<<<(f.n_rays + 255) / 256, 256, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
 }
 
 }  // namespace r360

@@ -52,12 +52,28 @@ struct ChunkBuffers {
   // first kHitCap hits of every ray, kept by k_count so that k_emit re-walks only the rays with more
   float2* hit_t;         // [kHitCap][n_rays] (t_in, delta)
   uint16_t* hit_lab;     // [kHitCap][n_rays]
+  // wavefront passes only (r360_set_wavefront; null otherwise):
+  uint32_t* pass_cnt;    // [n_rays] segments of the ray in the current pass
+  uint32_t* pass_off;    // [n_rays] first ray-major slot of the ray in the current pass
+  float4* st_c;          // [n_rays] compositing state carried between passes: C_r, C_g, C_b, D
+  float* st_T;           // [n_rays] transmittance carried between passes; < 0 = the ray is finished
   // tensor path only (null otherwise):
   uint4* dirblk;         // [n_rays*4] per ray: [1, 1, F(d), 0..] as 32 bf16 (pe.cuh)
   uint4* rec_dir;        // [G] binned like recs: (d.x, d.y, d.z, pose index)
 };
 
 constexpr int kSamplerThreads = 256;
+
+// Wavefronted early termination: the hits of a ray are fed to the MLP in passes
+// [h0, h1) = [0,2) [2,6) [6,16) [16,kHitCap) [kHitCap, inf); after every pass the compositing kernel retires
+// the rays whose transmittance fell below tau, so their remaining samples never reach the MLP.  The passes
+// inside the hit buffer replay it; the tail pass walks again (only rays still alive with more hits than the
+// buffer holds).  All zero in the single-pass path.
+struct PassParams {
+  int wavefront;
+  int first, last;
+  uint32_t h0, h1;
+};
 constexpr int kHitCap = 64;
 constexpr int kBlkListCap = 256;
 
@@ -65,7 +81,10 @@ void launch_count(const GridParams& g, const uint16_t* grid, const FrameParams& 
                   int n_bins, cudaStream_t s);
 void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_tile, cudaStream_t s);
 void launch_emit(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
-                 int n_bins, cudaStream_t s);
+                 int n_bins, const PassParams& pp, cudaStream_t s);
+// wavefront: segments of every ray in this pass, block-local offsets, the pass's histogram and reservations
+void launch_pass_count(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
+                       int n_bins, const PassParams& pp, cudaStream_t s);
 // fp32 MLP on the FP32 ALUs.  weights_t: per subfield, per layer W^T[in][out] then b[out].
 cudaError_t launch_mlp_fp32(const GridParams& g, const FrameParams& f, const ChunkBuffers& b,
                             const NetShape& net, const Fp32Layout& lay, const float* weights_t,
@@ -77,7 +96,7 @@ cudaError_t launch_mlp_tc(const GridParams& g, const FrameParams& f, const Chunk
                           const SubfieldFrame* frames, int n_bins, int segs_per_tile, int n_sms,
                           cudaStream_t s);
 void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
-                      float* out_rgb, float* out_depth, cudaStream_t s);
+                      float* out_rgb, float* out_depth, const PassParams& pp, cudaStream_t s);
 // debug: expand binned records into ray-major per-sample t and subfield id
 void launch_export_samples(const GridParams& g, const ChunkBuffers& b, int n_bins, unsigned n_segs,
                            float* t, int32_t* subfield, cudaStream_t s);

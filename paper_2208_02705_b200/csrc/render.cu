@@ -91,9 +91,11 @@ r360_scene::ChunkEvents* chunk_events(r360_scene* sc, unsigned idx) {
   return &sc->events[idx];
 }
 
-// Steps a1-a5 for one chunk: count, scan, (sync for the segment total), emit.
+// Steps a1-a5 for one chunk: count, scan, (sync for the segment total), emit.  pp.wavefront: one pass of the
+// wavefronted path -- the walk (k_count) runs with the first pass only, every pass bins its own hit range.
 r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::ChunkEvents* ev,
-                         unsigned long long& n_segs, unsigned long long& n_tiles, unsigned& launches) {
+                         unsigned long long& n_segs, unsigned long long& n_tiles, unsigned& launches,
+                         const PassParams& pp) {
   const int n = sc->desc.n_subfields;
   const size_t n_blocks = (f.n_rays + kSamplerThreads - 1) / kSamplerThreads;
   r360_status st;
@@ -111,16 +113,31 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
   cudaStream_t s = sc->stream;
   if ((st = grow(sc->buf.blk_list, sc->blk_list_cap, n_blocks * kBlkListCap, 1, 1)) != R360_OK) return st;
   if ((st = grow(sc->buf.blk_list_n, sc->blk_list_n_cap, n_blocks, 1, 1)) != R360_OK) return st;
+  sc->buf.pass_cnt = nullptr;
+  if (pp.wavefront) {
+    if ((st = grow(sc->d_pass_cnt, sc->pass_cnt_cap, f.n_rays, 1, 1)) != R360_OK) return st;
+    if ((st = grow(sc->buf.pass_off, sc->pass_off_cap, f.n_rays, 1, 1)) != R360_OK) return st;
+    if ((st = grow(sc->buf.st_c, sc->st_c_cap, f.n_rays, 1, 1)) != R360_OK) return st;
+    if ((st = grow(sc->buf.st_T, sc->st_T_cap, f.n_rays, 1, 1)) != R360_OK) return st;
+    sc->buf.pass_cnt = sc->d_pass_cnt;
+  }
   R360_CUDA(cudaMemsetAsync(sc->buf.bin_cnt, 0, (size_t)n * 4, s));
   R360_CUDA(cudaMemsetAsync(sc->buf.bin_ovf, 0, (size_t)n * 4, s));
   if (ev) cudaEventRecord(ev->e[0], s);
-  launch_count(sc->grid_p, sc->d_grid, f, sc->buf, n, s);
+  if (!pp.wavefront || pp.first) {
+    launch_count(sc->grid_p, sc->d_grid, f, sc->buf, n, s);
+    launches += 1;
+  }
+  if (pp.wavefront) {
+    launch_pass_count(sc->grid_p, sc->d_grid, f, sc->buf, n, pp, s);
+    launches += 1;
+  }
   if (ev) cudaEventRecord(ev->e[1], s);
   launch_scan(sc->buf, (int)n_blocks, n, sc->segs_per_tile, s);
   if (ev) cudaEventRecord(ev->e[2], s);
-  launches += 2;
+  launches += 1;
   R360_CUDA(cudaGetLastError());
-  R360_CUDA(cudaMemcpyAsync(sc->h_totals, sc->buf.totals, 2 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
+  R360_CUDA(cudaMemcpyAsync(sc->h_totals, sc->buf.totals, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
   R360_CUDA(cudaStreamSynchronize(s));
   n_segs = sc->h_totals[0];
   n_tiles = sc->h_totals[1];
@@ -134,7 +151,7 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
       if ((st = grow(sc->d_rec_dir, sc->rec_dir_cap, n_segs)) != R360_OK) return st;
       sc->buf.rec_dir = sc->d_rec_dir;
     }
-    launch_emit(sc->grid_p, sc->d_grid, f, sc->buf, n, s);
+    launch_emit(sc->grid_p, sc->d_grid, f, sc->buf, n, pp, s);
     launches += 1;
     R360_CUDA(cudaGetLastError());
   }
@@ -164,30 +181,46 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
     unsigned n_rays = (unsigned)((total_rays - ray0 < chunk) ? (total_rays - ray0) : chunk);
     FrameParams f = frame_params(sc, W, H, ray0, n_rays);
     r360_scene::ChunkEvents* ev = chunk_events(sc, chunk_idx);
-    unsigned long long n_segs = 0, n_tiles = 0;
-    if ((st = sample_chunk(sc, f, ev, n_segs, n_tiles, launches)) != R360_OK) return st;
-    if (n_segs) {
-      // per-sample MLP outputs: K * segments float4, ray-major
-      if ((st = grow(sc->buf.out, sc->out_cap, (size_t)n_segs * sc->grid_p.K)) != R360_OK) return st;
-      cudaError_t e;
-      if (sc->precision == 1)
-        e = launch_mlp_tc(sc->grid_p, f, sc->buf, sc->net, sc->d_wpack, sc->wpack_stride, sc->d_frames,
-                          sc->desc.n_subfields, sc->segs_per_tile, sc->n_sms, s);
-      else
-        e = launch_mlp_fp32(sc->grid_p, f, sc->buf, sc->net, sc->lay, sc->d_wt, sc->d_frames,
+    // single pass over all hits, or the wavefront passes (kernels.h: PassParams)
+    static const uint32_t kPassEnd[5] = {2, 6, 16, (uint32_t)kHitCap, 0xFFFFFFFFu};
+    const int n_pass = sc->wavefront ? 5 : 1;
+    for (int p = 0; p < n_pass; ++p) {
+      PassParams pp{};
+      if (sc->wavefront) {
+        pp.wavefront = 1;
+        pp.first = p == 0;
+        pp.last = p == n_pass - 1;
+        pp.h0 = p ? kPassEnd[p - 1] : 0;
+        pp.h1 = kPassEnd[p];
+      }
+      r360_scene::ChunkEvents* pev = p == 0 ? ev : nullptr;   // stage times: first pass only
+      unsigned long long n_segs = 0, n_tiles = 0;
+      if ((st = sample_chunk(sc, f, pev, n_segs, n_tiles, launches, pp)) != R360_OK) return st;
+      if (p > 0 && n_segs == 0) break;                       // every ray has finished
+      if (n_segs) {
+        // per-sample MLP outputs: K * segments float4, ray-major
+        if ((st = grow(sc->buf.out, sc->out_cap, (size_t)n_segs * sc->grid_p.K)) != R360_OK) return st;
+        cudaError_t e;
+        if (sc->precision == 1)
+          e = launch_mlp_tc(sc->grid_p, f, sc->buf, sc->net, sc->d_wpack, sc->wpack_stride, sc->d_frames,
                             sc->desc.n_subfields, sc->segs_per_tile, sc->n_sms, s);
-      if (e != cudaSuccess) return r360_cuda_fail(e, "launch_mlp");
+        else
+          e = launch_mlp_fp32(sc->grid_p, f, sc->buf, sc->net, sc->lay, sc->d_wt, sc->d_frames,
+                              sc->desc.n_subfields, sc->segs_per_tile, sc->n_sms, s);
+        if (e != cudaSuccess) return r360_cuda_fail(e, "launch_mlp");
+        launches += 1;
+      }
+      if (pev) cudaEventRecord(pev->e[4], s);
+      launch_composite(sc->grid_p, f, sc->buf, sc->desc.t_threshold, out_rgb, out_depth, pp, s);
       launches += 1;
+      R360_CUDA(cudaGetLastError());
+      if (pev) cudaEventRecord(pev->e[5], s);
+      stats.segments += n_segs;
+      stats.mlp_tiles += n_tiles;
     }
-    if (ev) cudaEventRecord(ev->e[4], s);
-    launch_composite(sc->grid_p, f, sc->buf, sc->desc.t_threshold, out_rgb, out_depth, s);
-    launches += 1;
-    R360_CUDA(cudaGetLastError());
-    if (ev) cudaEventRecord(ev->e[5], s);
-    stats.segments += n_segs;
-    stats.mlp_tiles += n_tiles;
   }
-  stats.samples_emitted = stats.segments * (uint64_t)sc->grid_p.K;
+  // wavefront: `segments` counts what reached the MLP; the geometric total comes from the walk
+  stats.samples_emitted = (sc->wavefront ? (uint64_t)sc->h_totals[3] : stats.segments) * (uint64_t)sc->grid_p.K;
   stats.chunks = chunk_idx;
   stats.kernel_launches = launches;
   sc->chunks_last = chunk_idx;
@@ -230,6 +263,12 @@ r360_status r360_set_precision(r360_scene* sc, int32_t mode) {
   if (!sc || (mode != 0 && mode != 1)) return R360_ERR_INVALID_ARG;
   if (mode == 1 && !sc->d_wpack) return R360_ERR_INVALID_ARG;
   sc->precision = mode;
+  return R360_OK;
+}
+
+r360_status r360_set_wavefront(r360_scene* sc, int32_t enable) {
+  if (!sc || (enable != 0 && enable != 1)) return R360_ERR_INVALID_ARG;
+  sc->wavefront = enable;
   return R360_OK;
 }
 
@@ -287,7 +326,7 @@ r360_status r360_debug_samples(r360_scene* sc, const float pose[12], int32_t W, 
   FrameParams f = frame_params(sc, W, H, 0, (unsigned)((long long)W * H));
   unsigned long long n_segs = 0, n_tiles = 0;
   unsigned launches = 0;
-  if ((st = sample_chunk(sc, f, nullptr, n_segs, n_tiles, launches)) != R360_OK) return st;
+  if ((st = sample_chunk(sc, f, nullptr, n_segs, n_tiles, launches, PassParams{})) != R360_OK) return st;
   *total = n_segs * (uint64_t)sc->grid_p.K;
   launch_export_counts(sc->buf, f.n_rays, sc->grid_p.K, counts, offsets, sc->stream);
   R360_CUDA(cudaGetLastError());

@@ -45,6 +45,40 @@ __device__ __forceinline__ uint32_t block_exclusive_scan(uint32_t x, uint32_t* w
   return warp_sums[wid] + incl - x;
 }
 
+// The block's bin reservations (made by k_count, or by k_pass_count for a wavefront pass) as shared-memory
+// cursors: cur[k] = next position of this block inside bin k, kNotReserved if the block reserved nothing.
+constexpr uint32_t kNotReserved = 0xFFFFFFFFu;
+
+__device__ __forceinline__ void load_reservations(const ChunkBuffers& b, uint32_t* cur, int n_bins) {
+  for (int k = threadIdx.x; k < n_bins; k += blockDim.x) cur[k] = kNotReserved;
+  __syncthreads();
+  const uint2* list = b.blk_list + (size_t)blockIdx.x * kBlkListCap;
+  const uint32_t n = b.blk_list_n[blockIdx.x];
+  for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
+    const uint2 e = list[i];
+    cur[e.x] = __ldg(b.bin_start + e.x) + e.y;
+  }
+  __syncthreads();
+}
+
+// The block's histogram -> one returning atomic per subfield present, remembered in the block's list.
+__device__ __forceinline__ void reserve_bins(const ChunkBuffers& b, const uint32_t* hist, int n_bins) {
+  __shared__ uint32_t list_n;
+  if (threadIdx.x == 0) list_n = 0;
+  __syncthreads();
+  uint2* list = b.blk_list + (size_t)blockIdx.x * kBlkListCap;
+  for (int k = threadIdx.x; k < n_bins; k += blockDim.x) {
+    const uint32_t c = hist[k];
+    if (c) {
+      const uint32_t i = atomicAdd(&list_n, 1u);
+      if (i < (uint32_t)kBlkListCap) list[i] = make_uint2((uint32_t)k, atomicAdd(&b.bin_cnt[k], c));
+      else atomicAdd(&b.bin_ovf[k], c);          // list full: k_emit falls back to the global cursor
+    }
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) b.blk_list_n[blockIdx.x] = min(list_n, (uint32_t)kBlkListCap);
+}
+
 // ---------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(kSamplerThreads)
 k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuffers b, int n_bins,
@@ -79,11 +113,13 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
         b.hit_lab[h] = (uint16_t)lab;
       }
       ++cnt;
-      unsigned peers = __match_any_sync(m, lab);
-      if ((peers & lanemask_lt()) == 0) {
-        uint32_t c = __popc(peers);
-        if (use_smem_hist) atomicAdd(&hist[lab], c);
-        else atomicAdd(&b.bin_ovf[lab], c);
+      if (!b.pass_cnt) {      // (wavefront: every pass builds its own histogram, k_pass_count)
+        unsigned peers = __match_any_sync(m, lab);
+        if ((peers & lanemask_lt()) == 0) {
+          uint32_t c = __popc(peers);
+          if (use_smem_hist) atomicAdd(&hist[lab], c);
+          else atomicAdd(&b.bin_ovf[lab], c);
+        }
       }
     }
   }
@@ -94,24 +130,16 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
     b.ray_off[r] = off;
   }
   if (threadIdx.x == 0) b.block_sum[blockIdx.x] = total;
+  if (b.pass_cnt) {
+    if (threadIdx.x == 0 && total) atomicAdd(&b.totals[3], (unsigned long long)total);   // geometric segments
+    return;
+  }
   if (use_smem_hist) {
     // The block RESERVES its share of every bin it touched: one returning atomic per (block, subfield),
     // remembered in the block's list, so that k_emit places this block's segments with shared-memory
     // cursors and no global atomics (thousands of warps hit the same few subfields at the same time).
-    __shared__ uint32_t list_n;
-    if (threadIdx.x == 0) list_n = 0;
     __syncthreads();
-    uint2* list = b.blk_list + (size_t)blockIdx.x * kBlkListCap;
-    for (int k = threadIdx.x; k < n_bins; k += blockDim.x) {
-      const uint32_t c = hist[k];
-      if (c) {
-        const uint32_t i = atomicAdd(&list_n, 1u);
-        if (i < (uint32_t)kBlkListCap) list[i] = make_uint2((uint32_t)k, atomicAdd(&b.bin_cnt[k], c));
-        else atomicAdd(&b.bin_ovf[k], c);          // list full: k_emit falls back to the global cursor
-      }
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) b.blk_list_n[blockIdx.x] = min(list_n, (uint32_t)kBlkListCap);
+    reserve_bins(b, hist, n_bins);
   } else if (threadIdx.x == 0) {
     b.blk_list_n[blockIdx.x] = 0;
   }
@@ -183,45 +211,112 @@ k_scan(ChunkBuffers b, int n_blocks, int n_bins, int segs_per_tile) {
 }
 
 // ---------------------------------------------------------------------------------------
+// ---------------------------------------------------------------------------------------
+// Wavefront pass: how many segments each ray contributes to this pass, block-local offsets, and the pass's
+// histogram / reservations.  Passes inside the hit buffer read the labels from it; the tail pass (hits beyond
+// the buffer, rays still alive only) walks again and skips the buffered hits.
 __global__ void __launch_bounds__(kSamplerThreads)
-k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuffers b, int n_bins,
-       int use_smem_cursor) {
-  extern __shared__ uint32_t cur[];      // [n_bins] when use_smem_cursor: next position of this block in each bin
-  constexpr uint32_t kNotReserved = 0xFFFFFFFFu;
-  if (use_smem_cursor) {
-    for (int k = threadIdx.x; k < n_bins; k += blockDim.x) cur[k] = kNotReserved;
-    __syncthreads();
-    const uint2* list = b.blk_list + (size_t)blockIdx.x * kBlkListCap;
-    const uint32_t n = b.blk_list_n[blockIdx.x];
-    for (uint32_t i = threadIdx.x; i < n; i += blockDim.x) {
-      const uint2 e = list[i];
-      cur[e.x] = __ldg(b.bin_start + e.x) + e.y;
-    }
+k_pass_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuffers b, int n_bins,
+             int use_smem_hist, PassParams pp) {
+  extern __shared__ uint32_t hist[];
+  __shared__ uint32_t warp_sums[33];
+  if (use_smem_hist) {
+    for (int k = threadIdx.x; k < n_bins; k += blockDim.x) hist[k] = 0;
     __syncthreads();
   }
+  const unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool tail = pp.h0 >= (uint32_t)kHitCap;
+  uint32_t m = 0;                      // segments of this ray in this pass
+  if (r < f.n_rays) {
+    const uint32_t cnt = b.ray_cnt[r];
+    if ((pp.first || b.st_T[r] >= 0.0f) && cnt > pp.h0) m = min(cnt, pp.h1) - pp.h0;
+    b.pass_cnt[r] = m;
+  }
+  uint32_t total;
+  const uint32_t off = block_exclusive_scan(m, warp_sums, total);
+  if (r < f.n_rays) b.ray_off[r] = off;
+  if (threadIdx.x == 0) b.block_sum[blockIdx.x] = total;
+  auto tally = [&](bool hit, uint32_t lab) {
+    const unsigned msk = __ballot_sync(0xffffffffu, hit);
+    if (hit) {
+      const unsigned peers = __match_any_sync(msk, lab);
+      if ((peers & lanemask_lt()) == 0) {
+        const uint32_t c = __popc(peers);
+        if (use_smem_hist) atomicAdd(&hist[lab], c);
+        else atomicAdd(&b.bin_ovf[lab], c);
+      }
+    }
+  };
+  if (!tail) {
+    uint32_t m_max = m;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m_max = max(m_max, __shfl_xor_sync(0xffffffffu, m_max, o));
+    for (uint32_t h = 0; h < m_max; ++h) {
+      const bool hit = h < m;
+      tally(hit, hit ? (uint32_t)b.hit_lab[(size_t)(pp.h0 + h) * f.n_rays + r] : 0u);
+    }
+  } else {
+    Walker w;
+    w.alive = false;
+    if (m) w.init(g, make_ray(f, r));
+    uint32_t seen = 0;
+    while (__any_sync(0xffffffffu, w.alive)) {
+      uint32_t lab = 0;
+      float t_in, t_out;
+      bool hit = w.next(g, grid, lab, t_in, t_out);
+      if (hit && seen++ < (uint32_t)kHitCap) hit = false;      // already processed from the hit buffer
+      tally(hit, lab);
+    }
+  }
+  if (use_smem_hist) {
+    __syncthreads();
+    reserve_bins(b, hist, n_bins);
+  } else if (threadIdx.x == 0) {
+    b.blk_list_n[blockIdx.x] = 0;
+  }
+}
+
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kSamplerThreads)
+k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuffers b, int n_bins,
+       int use_smem_cursor, PassParams pp) {
+  extern __shared__ uint32_t cur[];      // [n_bins] when use_smem_cursor: next position of this block in each bin
+  if (use_smem_cursor) load_reservations(b, cur, n_bins);
   const unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = r < f.n_rays;
   Walker w;
   w.alive = false;
-  uint32_t slot = 0, cnt = 0, h = 0;
+  uint32_t slot = 0, cnt = 0, h = 0, h_end = 0, skip = 0;
   uint4 dir = make_uint4(0, 0, 0, 0);
-  bool replay = false;
+  bool replay = true;
   if (valid) {
-    const Ray ray = make_ray(f, r);
-    dir = make_uint4(__float_as_uint(ray.d[0]), __float_as_uint(ray.d[1]), __float_as_uint(ray.d[2]), ray.pose);
+    const uint32_t cnt_total = b.ray_cnt[r];
+    cnt = pp.wavefront ? b.pass_cnt[r] : cnt_total;      // segments of this ray in this launch
     slot = b.block_sum[blockIdx.x] + b.ray_off[r];
-    b.ray_off[r] = slot;                 // now the global ray-major offset
-    cnt = b.ray_cnt[r];
-    replay = cnt <= kHitCap;             // every hit of this ray is in the hit buffer
-    if (!replay) w.init(g, ray);         // otherwise walk again
+    if (pp.wavefront) b.pass_off[r] = slot;
+    else b.ray_off[r] = slot;                              // now the global ray-major offset
+    // single pass: replay if every hit of the ray is in the hit buffer, otherwise walk again; wavefront: the
+    // passes inside the hit buffer replay, the tail pass walks and skips the buffered hits
+    replay = pp.wavefront ? pp.h0 < (uint32_t)kHitCap : cnt_total <= (uint32_t)kHitCap;
+    if (pp.wavefront && !replay) skip = kHitCap;
+    if (cnt) {
+      const Ray ray = make_ray(f, r);
+      dir = make_uint4(__float_as_uint(ray.d[0]), __float_as_uint(ray.d[1]), __float_as_uint(ray.d[2]), ray.pose);
+      if (replay) {
+        h = pp.wavefront ? pp.h0 : 0u;
+        h_end = h + cnt;
+      } else {
+        w.init(g, ray);                                    // otherwise walk again, all hits in one go
+      }
+    }
   }
-  bool more = replay ? cnt > 0 : w.alive;
+  bool more = replay ? h < h_end : w.alive;
   while (__any_sync(0xffffffffu, more)) {
     uint32_t lab = 0;
     float t_in = 0.f, dt = 0.f;
     bool hit = false;
     if (replay) {
-      if (h < cnt) {
+      if (h < h_end) {
         const size_t i = (size_t)h * f.n_rays + r;
         const float2 td = b.hit_t[i];
         t_in = td.x; dt = td.y;
@@ -229,10 +324,14 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
         hit = true;
         ++h;
       }
-      more = h < cnt;
+      more = h < h_end;
     } else {
       float t_out = 0.f;
       hit = w.next(g, grid, lab, t_in, t_out);
+      if (hit && skip) {                                   // tail pass: this hit was processed from the buffer
+        --skip;
+        hit = false;
+      }
       if (hit) dt = __fdiv_rn(__fsub_rn(t_out, t_in), g.Kf);    // reading D
       more = w.alive;
     }
@@ -243,7 +342,7 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
       uint32_t base = 0;
       if ((int)(threadIdx.x & 31) == leader) {
         const uint32_t c = (uint32_t)__popc(peers);
-        if (use_smem_cursor && cur[lab] != kNotReserved) base = atomicAdd(&cur[lab], c);   // reserved by k_count
+        if (use_smem_cursor && cur[lab] != kNotReserved) base = atomicAdd(&cur[lab], c);   // reserved by the block
         else base = __ldg(b.bin_start + lab) + atomicAdd(&b.bin_cursor[lab], c);
       }
       base = __shfl_sync(peers, base, leader);
@@ -299,11 +398,19 @@ void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_t
 }
 
 void launch_emit(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
-                 int n_bins, cudaStream_t s) {
+                 int n_bins, const PassParams& pp, cudaStream_t s) {
   int blocks = (f.n_rays + kSamplerThreads - 1) / kSamplerThreads;
   int use_smem = n_bins <= 8192;
   size_t smem = use_smem ? (size_t)n_bins * sizeof(uint32_t) : 0;
-  k_emit<<<blocks, kSamplerThreads, smem, s>>>(g, grid, f, b, n_bins, use_smem);
+  k_emit<<<blocks, kSamplerThreads, smem, s>>>(g, grid, f, b, n_bins, use_smem, pp);
+}
+
+void launch_pass_count(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
+                       int n_bins, const PassParams& pp, cudaStream_t s) {
+  int blocks = (f.n_rays + kSamplerThreads - 1) / kSamplerThreads;
+  int use_smem = n_bins <= 8192;
+  size_t smem = use_smem ? (size_t)n_bins * sizeof(uint32_t) : 0;
+  k_pass_count<<<blocks, kSamplerThreads, smem, s>>>(g, grid, f, b, n_bins, use_smem, pp);
 }
 
 void launch_export_samples(const GridParams& g, const ChunkBuffers& b, int n_bins, unsigned n_segs,

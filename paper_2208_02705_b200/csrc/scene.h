@@ -42,6 +42,9 @@ struct r360_scene {
   // configuration
   cudaStream_t stream = nullptr;
   int precision = 0;
+  int wavefront = 0;                        // r360_set_wavefront: feed the MLP in passes, retire finished rays between them
+  uint32_t* d_pass_cnt = nullptr;           // owned; buf.pass_cnt points here only during wavefront passes
+  size_t pass_cnt_cap = 0, pass_off_cap = 0, st_c_cap = 0, st_T_cap = 0;
   long long chunk_rays = 4ll << 20;
   // statistics of the last call
   struct ChunkEvents { cudaEvent_t e[6]; };
