@@ -230,3 +230,53 @@ def test_pinhole_view(r360, oracle, config, W, H, f):
         gpu.set_camera("pinhole", -1.0, 1.0, 0.0, 0.0)
     gpu.close()
     ora.close()
+
+
+def test_more_subfields_than_the_shared_memory_histogram_holds(r360, oracle):
+    """n_subfields > 8192: the sampler's per-block histograms and cursors do not fit shared memory and every bin
+    update goes through the global counters (bin_ovf / bin_cursor).  Samples bit-exact, fp32 and bf16 images within
+    their bars, wavefront passes identical to the single pass."""
+    from scenegen import mlp_param_count, weight_layout
+    sc = get_scene(1)
+    n = 8200
+    occ = np.asarray(sc.occupancy).reshape(-1) >= sc.occ_threshold
+    lab = np.asarray(sc.voxel_subfield).reshape(-1).copy()
+    v = np.flatnonzero(occ)
+    lab[v] = (lab[v].astype(np.int64) * 512 + v % 512) % n
+    rng = np.random.default_rng(77)
+    parts = []
+    for name, fo, fi in weight_layout(sc.hidden_width, sc.n_hidden):
+        a = np.sqrt(6.0 / (fi + fo))
+        parts.append(rng.uniform(-a, a, (n, fo * fi)))
+        parts.append(np.full((n, fo), 1.0 if name == "density" else 0.0))
+    w = np.concatenate(parts, 1).astype(F).reshape(-1)
+    assert w.size == n * mlp_param_count(sc.hidden_width, sc.n_hidden)
+    over = dict(n_subfields=n, voxel_subfield=lab, weights=w)
+    gpu = r360.scene_from(sc, **over)
+    okw = dict(dims=sc.dims, box_min=sc.box_min, box_max=sc.box_max, hidden_width=sc.hidden_width,
+               n_hidden=sc.n_hidden, pe_pos_levels=sc.pe_pos_levels, pe_dir_levels=sc.pe_dir_levels,
+               samples_per_voxel=sc.samples_per_voxel, t_threshold=sc.t_threshold,
+               density_activation=sc.density_activation, occ_threshold=sc.occ_threshold, occupancy=sc.occupancy, **over)
+    ora = oracle.scene(**okw)
+    pose, W, H = sc.poses[0], sc.W, sc.H
+    counts, offsets, t, sid = gpu.debug_samples(pose, W, H)
+    oc, ot, osid = ora.samples_rows(pose, W, H)
+    counts, offsets = counts.cpu().numpy().view(np.uint32), offsets.cpu().numpy().view(np.uint32)
+    assert np.array_equal(counts, oc)
+    idx = ray_major_index(counts, offsets)
+    assert np.array_equal(t.cpu().numpy().view(np.uint32)[idx], ot.view(np.uint32))
+    assert np.array_equal(sid.cpu().numpy()[idx], osid)
+    ref = ora.render_rows(pose, W, H)
+    rgb, depth = gpu.render(pose, W, H)
+    check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 1e-4)
+    gpu.set_wavefront(True)
+    rgb_w, depth_w = gpu.render(pose, W, H)
+    assert np.array_equal(rgb.cpu().numpy().view(np.uint32), rgb_w.cpu().numpy().view(np.uint32))
+    assert np.array_equal(depth.cpu().numpy().view(np.uint32), depth_w.cpu().numpy().view(np.uint32))
+    gpu.set_wavefront(False)
+    gpu.set_precision("bf16")
+    rgb, depth = gpu.render(pose, W, H)
+    t_max = float(np.linalg.norm(np.array(sc.box_max) - np.array(sc.box_min)))
+    check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 2e-3, amb_band=0.2, depth_tol=2e-3 * t_max)
+    gpu.close()
+    ora.close()
