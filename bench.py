@@ -328,6 +328,21 @@ def main():
             roof["executed_flop_per_sample"] = executed_flop_per_sample(sc.hidden_width, sc.n_hidden)
         roof["samples_per_launch"] = int(samples)
         roof["ms_per_launch"] = ms_mlp
+        # the memory-side stages against the measured HBM copy bandwidth: algorithmic bytes
+        rays, segs, Kk = W * H, int(st.segments), sc.samples_per_voxel
+        tensor = precision == "bf16"
+        stage_bytes = {
+            "k_count": rays * 8 + segs * 10 + (rays * 64 if tensor else 0),
+            "k_emit": rays * 8 + segs * 10 + segs * (40 if tensor else 24),
+            "k_composite": segs * Kk * 16 + segs * 8 + rays * 24,
+        }
+        stage_key = {"k_count": "ms_count", "k_emit": "ms_emit", "k_composite": "ms_composite"}
+        hbm_stages = {}
+        for kname, nbytes in stage_bytes.items():
+            ms_k = stage[stage_key[kname]] / args.steps
+            gbs = nbytes / (ms_k * 1e-3) / 1e9 if ms_k > 0 else 0.0
+            hbm_stages[kname] = {"algorithmic_bytes": int(nbytes), "ms": ms_k, "achieved_gbs": gbs,
+                                 "frac_of_hbm_peak": gbs / peaks["hbm"], "traffic": ncu_traffic(kname)}
         line = {"metric": "rays_per_second_equirect_render", "value": value, "unit": "rays/s", "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "bf16" if precision == "bf16" else "f32",
@@ -335,7 +350,7 @@ def main():
                 "fps": 1e3 / ms_step * world, "mlp_samples_per_s": samples / (ms_mlp * 1e-3),
                 "samples_per_frame": int(samples), "segments_per_frame": int(st.segments),
                 "stage_ms": {k: v / args.steps for k, v in stage.items()},
-                "clocks": clk, "roofline": roof,
+                "clocks": clk, "roofline": roof, "hbm_stages": hbm_stages,
                 "e2e": {"value": e2e_value, "unit": "rays/s", "h2d_bytes_per_step": 48 * world,
                         "d2h_bytes_per_step": W * H * 16 * world},
                 "gpu_launches": int(launches)}
