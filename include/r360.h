@@ -109,6 +109,20 @@ r360_status r360_assign_subfields(const int32_t dims[3], const float box_min[3],
                                   const uint8_t* occupancy, uint8_t occ_threshold, int32_t n,
                                   int32_t* labels_out);
 
+/* Floorplan estimation from the occupancy map (section 5.0.2; Fig. 6): the occupied voxels of
+ * the upper slice (default 60-65 % of the height) are projected to the floor plane, closed by a 3x3 square
+ * ("simple morphological operations"), the free region around the seed cell is segmented out with its inner
+ * boundary, and the occupied voxels of the lower slice (default 20-30 %) inside it are added as obstacles.
+ * Readings F1-F7 in DESIGN.md (height axis = z; a layer belongs to a slice iff its centre fraction lies in it;
+ * 4-connectivity).  Runs on the current CUDA device.  occupancy: HOST uint8[N] as in r360_scene_create;
+ * (seed_x, seed_y): a free cell inside the region to map (the viewer's position); upper / lower: {lo, hi}
+ * fractions of the height, or NULL for the paper's values; plan_out: HOST uint8[Ny*Nx], bit 0 interior, bit 1
+ * inner boundary, bit 2 obstacle (the floorplan of Fig. 6c = bits 1|2).  Caller owns all arrays.
+ * R360_ERR_INVALID_ARG: null pointers, bad dims, seed outside the image or on a wall cell, lo > hi. */
+r360_status r360_floorplan(const int32_t dims[3], const uint8_t* occupancy, uint8_t occ_threshold,
+                           int32_t seed_x, int32_t seed_y, const float upper[2], const float lower[2],
+                           uint8_t* plan_out);
+
 /* Camera of the following render / debug calls.  model 0 (default) = the equirectangular panorama of
  * Eq.2-3; model 1 = pinhole view for roaming (the paper's perspective display,
  * PAPER.md:206, :200, gives no model; reading P): pixel centre (i+0.5, j+0.5) ->

@@ -70,6 +70,9 @@ def lib():
     L.r360_assign_subfields.restype = C.c_int
     L.r360_assign_subfields.argtypes = [C.POINTER(C.c_int32), f32p, f32p, C.POINTER(C.c_uint8), C.c_uint8, i32,
                                         C.POINTER(C.c_int32)]
+    L.r360_floorplan.restype = C.c_int
+    L.r360_floorplan.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_uint8), C.c_uint8, i32, i32, f32p, f32p,
+                                 C.POINTER(C.c_uint8)]
     L.r360_set_wavefront.restype = C.c_int
     L.r360_set_wavefront.argtypes = [vp, i32]
     L.r360_set_camera.restype = C.c_int
@@ -128,6 +131,20 @@ def assign_subfields(occupancy, dims, box_min, box_max, occ_threshold, n):
     out = np.empty(occ.size, np.int32)
     _check(lib().r360_assign_subfields(d, lo, hi, occ.ctypes.data_as(C.POINTER(C.c_uint8)), int(occ_threshold),
                                        int(n), out.ctypes.data_as(C.POINTER(C.c_int32))), "r360_assign_subfields")
+    return out
+
+
+def floorplan(occupancy, dims, occ_threshold, seed_xy, upper=None, lower=None):
+    """Floorplan from the occupancy map on the GPU (r360_floorplan): uint8 [Ny][Nx], bit 0 interior, bit 1 inner
+    boundary, bit 2 obstacle."""
+    occ = np.ascontiguousarray(occupancy, np.uint8).reshape(-1)
+    d = (C.c_int32 * 3)(*[int(v) for v in dims])
+    assert occ.size == d[0] * d[1] * d[2]
+    up = (C.c_float * 2)(*upper) if upper is not None else None
+    lo = (C.c_float * 2)(*lower) if lower is not None else None
+    out = np.empty((d[1], d[0]), np.uint8)
+    _check(lib().r360_floorplan(d, occ.ctypes.data_as(C.POINTER(C.c_uint8)), int(occ_threshold), int(seed_xy[0]),
+                                int(seed_xy[1]), up, lo, out.ctypes.data_as(C.POINTER(C.c_uint8))), "r360_floorplan")
     return out
 
 
