@@ -78,7 +78,8 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
 /* Free a scene and all its device memory.  NULL is a no-op. */
 void r360_scene_destroy(r360_scene* scene);
 
-/* Render one W x H equirectangular view (Eq. 2-5; steps a1-a10 of DESIGN.md).
+/* Render one W x H view with the scene's camera (r360_set_camera; default: the equirectangular panorama of
+ * Eq. 2-3) -- Eq. 2-5; steps a1-a10 of DESIGN.md.
  *  pose       HOST float[12]: row-major 3x4 [R|o], camera (x right, y down, z forward,
  *             PAPER.md:84) -> world; o = camera centre.  Must be finite.
  *  out_rgb    DEVICE float[H*W*3], row-major, black background
