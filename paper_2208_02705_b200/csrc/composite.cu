@@ -6,7 +6,7 @@
 
 namespace r360 {
 
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(128)
 k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __restrict__ out_rgb,
             float* __restrict__ out_depth, PassParams pp) {
   const unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
@@ -79,7 +79,7 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __res
 
 void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
                       float* out_rgb, float* out_depth, const PassParams& pp, cudaStream_t s) {
-  k_composite<<<(f.n_rays + 255) / 256, 256, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
+  k_composite<<<(f.n_rays + 127) / 128, 128, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
 }
 
 }  // namespace r360
