@@ -41,9 +41,12 @@ struct FrameParams {
   const float* cos_theta;
 };
 
-// Binned segment record: one occupied voxel crossed by one ray (K samples).
-//   x = chunk-relative ray id, y = bits of t_in, z = bits of delta, w = ray-major segment slot
+// Binned segment record: one occupied voxel crossed by one ray (K samples), 32 bytes = two uint4:
+//   [0]: x = chunk-relative ray id, y = bits of t_in, z = bits of delta, w = ray-major segment slot
+//   [1]: bits of the ray direction d.x, d.y, d.z, and the pose index (so that the MLP kernels need no per-ray
+//        work and one address computation fetches everything a sample row needs)
 typedef uint4 SegRec;
+constexpr int kRecWords = 2;              // uint4 per record
 
 // ---------------------------------------------------------------------------------------
 // Ray of a pixel.  Eq.3 and reading B3: every operation individually

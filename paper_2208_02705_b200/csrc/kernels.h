@@ -47,7 +47,7 @@ struct ChunkBuffers {
   unsigned long long* totals;  // [4]: segments, tiles, samples_used (accumulated), spare
   float* seg_tin;        // [G] ray-major
   float* seg_dt;         // [G] ray-major
-  SegRec* recs;          // [G] binned by subfield
+  SegRec* recs;          // [G * kRecWords] binned by subfield (common.cuh: SegRec)
   float4* out;           // [G*K] (sigma, r, g, b) per sample, ray-major
   // first kHitCap hits of every ray, kept by k_count so that k_emit re-walks only the rays with more
   float2* hit_t;         // [kHitCap][n_rays] (t_in, delta)
@@ -59,7 +59,6 @@ struct ChunkBuffers {
   float* st_T;           // [n_rays] transmittance carried between passes; < 0 = the ray is finished
   // tensor path only (null otherwise):
   uint4* dirblk;         // [n_rays*4] per ray: [1, 1, F(d), 0..] as 32 bf16 (pe.cuh)
-  uint4* rec_dir;        // [G] binned like recs: (d.x, d.y, d.z, pose index)
 };
 
 constexpr int kSamplerThreads = 256;

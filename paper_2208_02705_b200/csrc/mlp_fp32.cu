@@ -84,7 +84,7 @@ k_mlp_fp32(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, Fp32Layout
     const int sidx = tid / K, j = tid - sidx * K;
     const bool active = (unsigned)sidx < nseg;
     SegRec rec = make_uint4(0, 0, 0, 0);
-    if (active) rec = b.recs[seg0 + sidx];
+    if (active) rec = b.recs[(size_t)(seg0 + sidx) * kRecWords];
     const float t_in = __uint_as_float(rec.y), dt = __uint_as_float(rec.z);
     const float t = __fmaf_rn((float)j + 0.5f, dt, t_in);            // reading D
     const Ray ray = make_ray(f, active ? rec.x : 0u);

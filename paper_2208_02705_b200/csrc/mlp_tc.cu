@@ -340,16 +340,16 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     SegRec rec = make_uint4(0, 0, 0, 0);
     uint4 rd = make_uint4(0, 0, 0, 0);
     if (active) {
-      rec = __ldg(b.recs + seg0 + sidx);
-      rd = __ldg(b.rec_dir + seg0 + sidx);                   // direction, pose
+      const SegRec* rp = b.recs + (size_t)(seg0 + sidx) * kRecWords;
+      rec = __ldg(rp);
+      rd = __ldg(rp + 1);                                    // direction, pose
     }
     if (j == 0) {
       // hide DRAM latency without registers: this tile's direction block (read after trunk-1 is
       // issued) and the next tile's records go to L2 now
       if (active) prefetch_l2(b.dirblk + (size_t)rec.x * 4);
       if (seg0 + spt + sidx < k_seg_end) {
-        prefetch_l2(b.recs + seg0 + spt + sidx);
-        prefetch_l2(b.rec_dir + seg0 + spt + sidx);
+        prefetch_l2(b.recs + (size_t)(seg0 + spt + sidx) * kRecWords);
       }
     }
     const float* P = f.poses + rd.w * 12;
@@ -447,7 +447,7 @@ static cudaError_t launch_tc_t(const GridParams& g, const FrameParams& f, const 
                                const NetShape& net, const void* wpack, const SubfieldFrame* frames, int n_bins,
                                int spt, int n_sms, cudaStream_t s) {
   using S = TcShape<WD>;
-  if (!b.dirblk || !b.rec_dir) return cudaErrorInvalidValue;
+  if (!b.dirblk) return cudaErrorInvalidValue;
   TcLayout lay = make_tc_layout<WD>(net.Hd);
   // one CTA per SM owns all 512 TMEM columns; asking for more than half of the shared memory keeps a
   // second CTA (which would block in tcgen05.alloc) off the SM

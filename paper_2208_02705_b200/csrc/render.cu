@@ -145,12 +145,7 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
   if (n_segs) {
     if ((st = grow(sc->buf.seg_tin, sc->seg_tin_cap, n_segs)) != R360_OK) return st;
     if ((st = grow(sc->buf.seg_dt, sc->seg_dt_cap, n_segs)) != R360_OK) return st;
-    if ((st = grow(sc->buf.recs, sc->recs_cap, n_segs)) != R360_OK) return st;
-    sc->buf.rec_dir = nullptr;
-    if (sc->precision == 1) {
-      if ((st = grow(sc->d_rec_dir, sc->rec_dir_cap, n_segs)) != R360_OK) return st;
-      sc->buf.rec_dir = sc->d_rec_dir;
-    }
+    if ((st = grow(sc->buf.recs, sc->recs_cap, n_segs * kRecWords)) != R360_OK) return st;
     launch_emit(sc->grid_p, sc->d_grid, f, sc->buf, n, pp, s);
     launches += 1;
     R360_CUDA(cudaGetLastError());

@@ -347,8 +347,8 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
       }
       base = __shfl_sync(peers, base, leader);
       uint32_t pos = base + __popc(peers & lanemask_lt());
-      b.recs[pos] = make_uint4(r, __float_as_uint(t_in), __float_as_uint(dt), slot);
-      if (b.rec_dir) b.rec_dir[pos] = dir;
+      b.recs[(size_t)pos * kRecWords] = make_uint4(r, __float_as_uint(t_in), __float_as_uint(dt), slot);
+      b.recs[(size_t)pos * kRecWords + 1] = dir;
       b.seg_tin[slot] = t_in;
       b.seg_dt[slot] = dt;
       ++slot;
@@ -368,7 +368,7 @@ __global__ void k_export_samples(GridParams g, ChunkBuffers b, int n_bins, unsig
     int mid = (lo + hi) >> 1;
     if (b.bin_start[mid] <= pos) lo = mid; else hi = mid;
   }
-  SegRec rec = b.recs[pos];
+  SegRec rec = b.recs[(size_t)pos * kRecWords];
   float t_in = __uint_as_float(rec.y), dt = __uint_as_float(rec.z);
   size_t s0 = (size_t)rec.w * g.K;
   for (int j = 0; j < g.K; ++j) {

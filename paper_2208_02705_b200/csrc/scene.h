@@ -31,9 +31,8 @@ struct r360_scene {
   // chunk buffers and capacities
   r360::ChunkBuffers buf{};
   size_t ray_cnt_cap = 0, ray_off_cap = 0, blocks_cap = 0;
-  size_t seg_tin_cap = 0, seg_dt_cap = 0, recs_cap = 0, out_cap = 0, dirblk_cap = 0, rec_dir_cap = 0, hit_t_cap = 0, hit_lab_cap = 0, blk_list_cap = 0, blk_list_n_cap = 0;
-  uint4* d_dirblk = nullptr;                // owned; buf.dirblk / buf.rec_dir point at these only while the
-  uint4* d_rec_dir = nullptr;               // tensor path is selected
+  size_t seg_tin_cap = 0, seg_dt_cap = 0, recs_cap = 0, out_cap = 0, dirblk_cap = 0, hit_t_cap = 0, hit_lab_cap = 0, blk_list_cap = 0, blk_list_n_cap = 0;
+  uint4* d_dirblk = nullptr;                // owned; buf.dirblk points here only while the tensor path is selected
   unsigned long long* h_totals = nullptr;   // pinned [4]
   // D2H staging for r360_render_batch_host
   float* d_stage_rgb = nullptr;
