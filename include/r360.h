@@ -124,6 +124,20 @@ r360_status r360_floorplan(const int32_t dims[3], const uint8_t* occupancy, uint
                            int32_t seed_x, int32_t seed_y, const float upper[2], const float lower[2],
                            uint8_t* plan_out);
 
+/* Progressive probabilistic occupancy, one observation (Eq. 6; Algorithm 1 stage I): a depth
+ * panorama (Eq. 4's radial distance) and optionally an uncertainty panorama seen from `pose` are fused into the
+ * log-odds grid, logit(p|z_1:t) = logit(p|z_1:t-1) + logit(p|z_t), clamped to [-2, 3.5] (:119-122).  Readings
+ * O1-O5 in DESIGN.md: Octomap's scan insertion and defaults (the framework the paper adopts; its default clamps
+ * are the paper's): a voxel holding the end point of a ray gets + ln(p/(1-p)), p = 0.5 + 0.2 (1 - u), u the smallest
+ * uncertainty in [0,1] of the rays ending there (0 without a map); a voxel only crossed before the end points gets
+ * ln(0.4/0.6); pixels with depth <= 0 or non-finite are skipped; a voxel is occupied iff logit > ln(0.97/0.03).
+ * Runs on the current CUDA device.  logodds: HOST float[N], read and written; pose: HOST float[12] as in
+ * r360_render; depth, uncertainty (may be NULL): HOST float[H*W] of a W x H equirectangular image.
+ * R360_ERR_INVALID_ARG: null pointers, bad dims/box, W or H < 1, non-finite pose. */
+r360_status r360_occupancy_fuse(const int32_t dims[3], const float box_min[3], const float box_max[3],
+                                float* logodds, const float pose[12], int32_t W, int32_t H,
+                                const float* depth, const float* uncertainty);
+
 /* Camera of the following render / debug calls.  model 0 (default) = the equirectangular panorama of
  * Eq.2-3; model 1 = pinhole view for roaming (the paper's perspective display,
  * PAPER.md:206, :200, gives no model; reading P): pixel centre (i+0.5, j+0.5) ->

@@ -70,6 +70,8 @@ def lib():
     L.r360_assign_subfields.restype = C.c_int
     L.r360_assign_subfields.argtypes = [C.POINTER(C.c_int32), f32p, f32p, C.POINTER(C.c_uint8), C.c_uint8, i32,
                                         C.POINTER(C.c_int32)]
+    L.r360_occupancy_fuse.restype = C.c_int
+    L.r360_occupancy_fuse.argtypes = [C.POINTER(C.c_int32), f32p, f32p, f32p, f32p, i32, i32, f32p, f32p]
     L.r360_floorplan.restype = C.c_int
     L.r360_floorplan.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_uint8), C.c_uint8, i32, i32, f32p, f32p,
                                  C.POINTER(C.c_uint8)]
@@ -132,6 +134,23 @@ def assign_subfields(occupancy, dims, box_min, box_max, occ_threshold, n):
     _check(lib().r360_assign_subfields(d, lo, hi, occ.ctypes.data_as(C.POINTER(C.c_uint8)), int(occ_threshold),
                                        int(n), out.ctypes.data_as(C.POINTER(C.c_int32))), "r360_assign_subfields")
     return out
+
+
+def occupancy_fuse(logodds, dims, box_min, box_max, pose, W, H, depth, uncertainty=None):
+    """One observation fused into the log-odds grid on the GPU (r360_occupancy_fuse); returns the new float32 grid."""
+    d = (C.c_int32 * 3)(*[int(v) for v in dims])
+    lo = (C.c_float * 3)(*[float(v) for v in box_min])
+    hi = (C.c_float * 3)(*[float(v) for v in box_max])
+    L = np.array(logodds, np.float32).reshape(-1).copy()
+    assert L.size == d[0] * d[1] * d[2]
+    fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
+    p = np.ascontiguousarray(pose, np.float32).reshape(12)
+    dep = np.ascontiguousarray(depth, np.float32).reshape(-1)
+    assert dep.size == W * H
+    unc = None if uncertainty is None else np.ascontiguousarray(uncertainty, np.float32).reshape(-1)
+    _check(lib().r360_occupancy_fuse(d, lo, hi, fp(L), fp(p), W, H, fp(dep), None if unc is None else fp(unc)),
+           "r360_occupancy_fuse")
+    return L
 
 
 def floorplan(occupancy, dims, occ_threshold, seed_xy, upper=None, lower=None):
