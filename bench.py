@@ -209,6 +209,41 @@ def time_config(r360, config, precision, steps=5, warmup=3, pinhole=None):
     return out
 
 
+def time_extras(r360, config):
+    """Wall-clock of the stand-alone entry points (host arrays in, host arrays out) on a BASELINE.json scene."""
+    import torch
+    from scenegen import make_scene
+    sc = make_scene(config, with_weights=False)
+    out = {}
+
+    def wall(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            r = fn()
+        torch.cuda.synchronize()
+        return (time.perf_counter() - t0) / reps, r
+
+    dt, lab = wall(lambda: r360.assign_subfields(sc.occupancy, sc.dims, sc.box_min, sc.box_max, sc.occ_threshold,
+                                                 sc.n_subfields), 2)
+    out["assign_subfields"] = {"seconds": dt, "occupied_voxels": int((lab >= 0).sum()), "n": sc.n_subfields,
+                               "what": "Algorithm 1 stage II (PAPER.md:147-154), r360_assign_subfields"}
+    pose = np.asarray(sc.poses[0], np.float64).reshape(3, 4)
+    vs = (np.array(sc.box_max) - np.array(sc.box_min)) / np.array(sc.dims)
+    cell = np.floor((pose[:, 3] - np.array(sc.box_min)) / vs).astype(int)
+    dt, plan = wall(lambda: r360.floorplan(sc.occupancy, sc.dims, sc.occ_threshold, (int(cell[0]), int(cell[1]))), 5)
+    out["floorplan"] = {"seconds": dt, "cells": int(plan.size), "interior_cells": int((plan & 1).sum()),
+                        "what": "floorplan estimation (PAPER.md:176-178), r360_floorplan"}
+    W, H = 1024, 512
+    depth = np.full((H, W), 2.5, np.float32)
+    L0 = np.zeros(int(np.prod(sc.dims)), np.float32)
+    dt, L = wall(lambda: r360.occupancy_fuse(L0, sc.dims, sc.box_min, sc.box_max, sc.poses[0], W, H, depth), 5)
+    out["occupancy_fuse"] = {"seconds": dt, "image": [W, H], "voxels": int(L0.size), "voxels_updated": int((L != 0).sum()),
+                             "what": "one observation of Eq. 6 (PAPER.md:117-128), r360_occupancy_fuse, synthetic depth"}
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -360,6 +395,7 @@ def main():
             line["other_configs"] = [time_config(r360, c, precision) for c in (1, 2, 4, 5) if c != args.config]
             # the paper times its perspective (roaming) view at 720p: same scene, 90 degree pinhole
             line["other_configs"].append(time_config(r360, args.config, precision, pinhole=(1280, 720, 640.0)))
+            line["extras"] = time_extras(r360, args.config)
         if not args.no_cpu_baseline:
             cb = oracle_sample(sc, args.ref_row_stride)
             line["cpu_baseline"] = {"value": cb["rays_per_s"], "unit": "rays/s", "cores": cb["cores"],
