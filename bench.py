@@ -267,7 +267,8 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     torch.cuda.set_device(local)
-    if world > 1:
+    use_dist = world > 1 or "TORCHELASTIC_RUN_ID" in os.environ      # under torchrun: always go through NCCL
+    if use_dist:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     import __graft_entry__ as g
     import paper_2208_02705_b200 as r360
@@ -294,7 +295,7 @@ def main():
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
 
     def barrier():
-        if world > 1:
+        if use_dist:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -320,7 +321,7 @@ def main():
     clk = clocks.stop()
     ms_total = sum(a.elapsed_time(b) for a, b in ev)
     tt = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if world > 1:
+    if use_dist:
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
     ms_step = float(tt.item()) / args.steps
     rays_step = W * H * world
@@ -338,7 +339,7 @@ def main():
         scene.render_batch_host(h_pose.numpy(), W, H, h_rgb.numpy(), h_depth.numpy())
     torch.cuda.synchronize()
     te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-    if world > 1:
+    if use_dist:
         dist.all_reduce(te, op=dist.ReduceOp.MAX)
     e2e_value = rays_step * args.steps / float(te.item())
 
@@ -401,7 +402,7 @@ def main():
             line["cpu_baseline"] = {"value": cb["rays_per_s"], "unit": "rays/s", "cores": cb["cores"],
                                     "kind": "oracle", "sample": cb["sample"]}
         print(json.dumps(line), flush=True)
-    if world > 1:
+    if use_dist:
         dist.destroy_process_group()
 
 
