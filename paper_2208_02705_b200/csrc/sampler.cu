@@ -1,11 +1,15 @@
-// r360 -- ray generation + occupancy DDA sampler, and the binning by subfield (steps a1-a5).
+// r360 -- ray generation + occupancy walk sampler, and the binning by subfield (steps a1-a5).
 //
-// Two walks per ray, no intermediate ray-major record stream:
-//   k_count : walk #1  -> segments per ray, block-local exclusive offsets, per-subfield histogram
-//   k_scan  : one launch, two blocks: exclusive scan of the block sums; exclusive scan of the
-//             histogram (bin starts) and of the per-subfield MLP tile counts
-//   k_emit  : walk #2  -> each segment goes straight to its bin (warp-aggregated cursor atomics);
-//             the ray-major (t_in, delta) pair is kept for the compositing kernel
+//   k_count : one walk per ray (exact empty-space skipping, common.cuh: Walker) -> segments per ray, block-local
+//             exclusive offsets, the first kHitCap hits of every ray in a ray-major hit buffer, the ray's direction
+//             block for the tensor path, the per-subfield histogram of the block and -- from it -- the block's
+//             RESERVATION of a range in every bin it touched (one returning atomic per block and subfield)
+//   k_scan  : one launch, two blocks: exclusive scan of the block sums; exclusive scan of the histogram (bin
+//             starts) and of the per-subfield MLP tile counts
+//   k_emit  : every segment goes to its bin: hits are replayed from the hit buffer and placed with shared-memory
+//             cursors inside the block's reservations (no global atomics); only rays with more than kHitCap hits
+//             walk again.  The ray-major (t_in, delta) pair is kept for the compositing kernel.
+//   k_pass_count : the histogram / reservation step of one wavefront pass (r360_set_wavefront), from the hit buffer
 // A "segment" is one occupied voxel crossed by one ray; it stands for K samples (reading D).
 // PAPER.md:174 (ray casting to localise occupied voxels, per-voxel tiny-MLP label), :164, :29.
 #include "kernels.h"
