@@ -233,6 +233,9 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   extern __shared__ __align__(128) unsigned char smem_all[];   // G weight buffers of lay.total bytes
   __shared__ __align__(8) uint64_t bar_w_s[G], bar_d_s[G];
   __shared__ uint32_t tmem_base_s;
+  // the NEXT tile's segment records, copied asynchronously while this tile runs (two buffers per group)
+  constexpr int kStageSegs = 32;                               // staging serves K >= 4 (at most 32 segments per tile)
+  __shared__ __align__(16) uint4 rec_stage_s[G][2][kStageSegs * kRecWords];
   // group and warp index are the same in every lane of a warp: broadcast from lane 0 so that everything derived
   // from them (TMEM columns, weight buffer, barriers, tile range) can live in uniform registers (measured: 5 %)
   const int grp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 7), 0);
@@ -306,7 +309,8 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   };
 
   unsigned k_tile_end = 0, k_tile_begin = 0, k_seg_begin = 0, k_seg_end = 0;
-  bool have_k = false;
+  bool have_k = false, staged = false;
+  int stage_buf = 0;
   SubfieldFrame fr = frames[0];
   for (unsigned tile = tile0; tile < tile1; ++tile) {
     if (tile >= k_tile_end || !have_k) {
@@ -340,18 +344,33 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     SegRec rec = make_uint4(0, 0, 0, 0);
     uint4 rd = make_uint4(0, 0, 0, 0);
     if (active) {
-      const SegRec* rp = b.recs + (size_t)(seg0 + sidx) * kRecWords;
-      rec = __ldg(rp);
-      rd = __ldg(rp + 1);                                    // direction, pose
-    }
-    if (j == 0) {
-      // hide DRAM latency without registers: this tile's direction block (read after trunk-1 is
-      // issued) and the next tile's records go to L2 now
-      if (active) prefetch_l2(b.dirblk + (size_t)rec.x * 4);
-      if (seg0 + spt + sidx < k_seg_end) {
-        prefetch_l2(b.recs + (size_t)(seg0 + spt + sidx) * kRecWords);
+      if (staged) {                                          // copied to shared memory during the previous tile
+        const uint4* sp = &rec_stage_s[grp][stage_buf][sidx * kRecWords];
+        rec = sp[0];
+        rd = sp[1];
+      } else {
+        const SegRec* rp = b.recs + (size_t)(seg0 + sidx) * kRecWords;
+        rec = __ldg(rp);
+        rd = __ldg(rp + 1);                                  // direction, pose
       }
     }
+    // hide DRAM latency without registers: this tile's direction block (read after trunk-1 is issued) goes to
+    // L2 now; the next tile's records (same subfield, so their place is known) travel to shared memory with
+    // cp.async and the records of the tile after it go to L2
+    const bool stage_next = spt <= kStageSegs && tile + 1 < tile1 && tile + 1 < k_tile_end;
+    if (j == 0) {
+      if (active) prefetch_l2(b.dirblk + (size_t)rec.x * 4);
+      const unsigned sn = seg0 + spt + sidx;
+      if (sn < k_seg_end) {
+        if (stage_next) {
+          uint4* dp = &rec_stage_s[grp][stage_buf ^ 1][sidx * kRecWords];
+          cp_async_16(dp, b.recs + (size_t)sn * kRecWords);
+          cp_async_16(dp + 1, b.recs + (size_t)sn * kRecWords + 1);
+        }
+        if (sn + spt < k_seg_end) prefetch_l2(b.recs + (size_t)(sn + spt) * kRecWords);
+      }
+    }
+    cp_async_commit();
     const float* P = f.poses + rd.w * 12;
     const float t = __fmaf_rn(jf, __uint_as_float(rec.z), __uint_as_float(rec.y));   // reading D
     float q[3];                                              // reading A3
@@ -412,7 +431,10 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     // ---- heads: rgb from the colour activation (takes the direction block's columns), density
     //      from h (still in place); both N = 16, accumulators side by side
     d_to_a(tA + S::A_FD);
+    cp_async_wait_all();                                     // the staged records are complete before this barrier
     publish();
+    staged = stage_next;
+    stage_buf ^= 1;
     if (warp == 0) {
       if (elect_one()) {
         fence_after_sync();
