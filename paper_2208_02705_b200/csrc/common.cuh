@@ -118,7 +118,8 @@ struct Walker {
   float o[3], d[3], inv[3];
   float t0, ti;     // clip distance; entry distance of the current voxel
   int idx[3];
-  bool neg[3], par[3];
+  int step[3], off[3];   // direction of travel per axis: step = +1 / -1, off = 1 / 0 (index offset of the far plane)
+  bool par[3];
   bool alive;
 
   __device__ __forceinline__ float t_at(const GridParams& g, int a, int k) const {
@@ -132,7 +133,8 @@ struct Walker {
       o[a] = ray.o[a];
       d[a] = ray.d[a];
       par[a] = fabsf(ray.d[a]) < kParallelEps;
-      neg[a] = ray.d[a] < 0.0f;
+      off[a] = ray.d[a] < 0.0f ? 0 : 1;
+      step[a] = 2 * off[a] - 1;
       inv[a] = par[a] ? 0.0f : __fdiv_rn(1.0f, ray.d[a]);
     }
     // C2: clip against the box
@@ -144,8 +146,8 @@ struct Walker {
       if (par[a]) {
         if (!(o[a] >= g.box_min[a] && o[a] < plane(g, a, N))) alive = false;
       } else {
-        float n_ = t_at(g, a, neg[a] ? N : 0);
-        float f_ = t_at(g, a, neg[a] ? 0 : N);
+        float n_ = t_at(g, a, off[a] ? 0 : N);
+        float f_ = t_at(g, a, off[a] ? N : 0);
         if (n_ > t0) t0 = n_;
         if (f_ < t1) t1 = f_;
       }
@@ -159,14 +161,17 @@ struct Walker {
       float f = floorf(__fdiv_rn(__fsub_rn(pa, g.box_min[a]), g.vs[a]));
       int N = g.dims[a];
       idx[a] = (f < 0.0f) ? 0 : ((f > (float)(N - 1)) ? N - 1 : (int)f);
-      if (!par[a]) ti = fmaxf(ti, t_at(g, a, idx[a] + (neg[a] ? 1 : 0)));
+      if (!par[a]) ti = fmaxf(ti, t_at(g, a, idx[a] + 1 - off[a]));
     }
+    // from here on a parallel axis never limits the walk: (plane - (-inf)) * 1 = +inf without a select
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+      if (par[a]) { o[a] = __int_as_float(0xff800000); inv[a] = 1.0f; }
   }
 
   // On true: lab = subfield label of the voxel, [t_in, t_out] its crossing interval.
   __device__ __forceinline__ bool next(const GridParams& g, const uint16_t* __restrict__ grid,
                                        uint32_t& lab, float& t_in, float& t_out) {
-    const float inf = __int_as_float(0x7f800000);
     while (alive) {
       const uint32_t l = __ldg(grid + (idx[2] * g.dims[1] + idx[1]) * g.dims[0] + idx[0]);
       const bool empty = l >= kEmptyBase;
@@ -176,8 +181,8 @@ struct Walker {
       float tf[3];
 #pragma unroll
       for (int a = 0; a < 3; ++a) {
-        kx[a] = neg[a] ? max(idx[a] - r, 0) : min(idx[a] + r + 1, g.dims[a]);
-        tf[a] = par[a] ? inf : t_at(g, a, kx[a]);
+        kx[a] = min(max(idx[a] + step[a] * r + off[a], 0), g.dims[a]);
+        tf[a] = t_at(g, a, kx[a]);
       }
       int amin = 2;
       float to = tf[2];
@@ -189,7 +194,7 @@ struct Walker {
 #pragma unroll
       for (int a = 0; a < 3; ++a) {
         if (a == amin) {
-          idx[a] = neg[a] ? kx[a] - 1 : kx[a];
+          idx[a] = kx[a] + off[a] - 1;
           if ((unsigned)idx[a] >= (unsigned)g.dims[a]) alive = false;
         }
       }
@@ -200,20 +205,20 @@ struct Walker {
         for (int a = 0; a < 3; ++a) {
           if (a != amin && !par[a] && alive) {
             const int lo = max(idx[a] - r, 0), hi = min(idx[a] + r, g.dims[a] - 1);
-            const int first = neg[a] ? hi : lo, step = neg[a] ? -1 : 1, off = neg[a] ? 0 : 1;
+            const int first = off[a] ? lo : hi;
             const float p = __fmaf_rn(to, d[a], o[a]);
             int gi = __float2int_rd((p - g.box_min[a]) * g.inv_vs[a]);     // guess, verified below
             gi = min(max(gi, lo), hi);
             // forward: the far plane of gi must lie beyond `to`
-            while (!(t_at(g, a, gi + off) > to)) {
-              gi += step;
+            while (!(t_at(g, a, gi + off[a]) > to)) {
+              gi += step[a];
               if ((unsigned)gi >= (unsigned)g.dims[a]) { alive = false; break; }
             }
             // backward: no earlier index of the cube may qualify; tn = near plane of gi
-            float tn = t_at(g, a, gi - step + off);
+            float tn = t_at(g, a, gi - step[a] + off[a]);
             while (gi != first && tn > to) {
-              gi -= step;
-              tn = t_at(g, a, gi - step + off);
+              gi -= step[a];
+              tn = t_at(g, a, gi - step[a] + off[a]);
             }
             idx[a] = gi;
             tin = fmaxf(tin, tn);
