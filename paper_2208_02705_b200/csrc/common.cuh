@@ -169,10 +169,11 @@ struct Walker {
       if (par[a]) { o[a] = __int_as_float(0xff800000); inv[a] = 1.0f; }
   }
 
-  // On true: lab = subfield label of the voxel, [t_in, t_out] its crossing interval.
-  __device__ __forceinline__ bool next(const GridParams& g, const uint16_t* __restrict__ grid,
+  // One iteration of the walk (the ray must be alive): on true the voxel just left was an occupied crossed voxel,
+  // lab = its subfield label, [t_in, t_out] its crossing interval.
+  __device__ __forceinline__ bool advance(const GridParams& g, const uint16_t* __restrict__ grid,
                                        uint32_t& lab, float& t_in, float& t_out) {
-    while (alive) {
+    {
       const uint32_t l = __ldg(grid + (idx[2] * g.dims[1] + idx[1]) * g.dims[0] + idx[0]);
       const bool empty = l >= kEmptyBase;
       const int r = empty ? (int)(l & 0xFFu) - 1 : 0;     // half-size of the empty cube (0: this voxel only)
@@ -228,8 +229,15 @@ struct Walker {
       } else {
         ti = fmaxf(ti, to);
       }
-      if (hit) return true;
+      return hit;
     }
+  }
+
+  // Advances to the next OCCUPIED crossed voxel; false when the ray has left the grid.
+  __device__ __forceinline__ bool next(const GridParams& g, const uint16_t* __restrict__ grid,
+                                       uint32_t& lab, float& t_in, float& t_out) {
+    while (alive)
+      if (advance(g, grid, lab, t_in, t_out)) return true;
     return false;
   }
 };

@@ -107,8 +107,11 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
   while (__any_sync(0xffffffffu, w.alive)) {
     uint32_t lab = 0;
     float t_in, t_out;
-    bool hit = w.next(g, grid, lab, t_in, t_out);
+    // one walk iteration per lane and round: a lane that has found a voxel goes on with the others instead of
+    // waiting for them to find theirs
+    const bool hit = w.alive && w.advance(g, grid, lab, t_in, t_out);
     unsigned m = __ballot_sync(0xffffffffu, hit);
+    if (m == 0) continue;
     if (hit) {
       if (cnt < kHitCap) {
         // reading D: delta = (t_out - t_in) / K, one subtract, one divide
@@ -267,7 +270,7 @@ k_pass_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, Chu
     while (__any_sync(0xffffffffu, w.alive)) {
       uint32_t lab = 0;
       float t_in, t_out;
-      bool hit = w.next(g, grid, lab, t_in, t_out);
+      bool hit = w.alive && w.advance(g, grid, lab, t_in, t_out);
       if (hit && seen++ < (uint32_t)kHitCap) hit = false;      // already processed from the hit buffer
       tally(hit, lab);
     }
@@ -331,7 +334,7 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
       more = h < h_end;
     } else {
       float t_out = 0.f;
-      hit = w.next(g, grid, lab, t_in, t_out);
+      hit = w.alive && w.advance(g, grid, lab, t_in, t_out);     // one walk iteration per round (see k_count)
       if (hit && skip) {                                   // tail pass: this hit was processed from the buffer
         --skip;
         hit = false;
