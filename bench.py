@@ -370,7 +370,7 @@ def main():
         stage_bytes = {
             "k_count": rays * 8 + segs * 10 + (rays * 64 if tensor else 0),
             "k_emit": rays * 8 + segs * 10 + segs * (40 if tensor else 24),
-            "k_composite": segs * Kk * 16 + segs * 8 + rays * 24,
+            "k_composite": segs * Kk * (8 if tensor else 16) + segs * 8 + rays * 24,   # tensor path: binary16 x4 per sample
         }
         stage_key = {"k_count": "ms_count", "k_emit": "ms_emit", "k_composite": "ms_composite"}
         hbm_stages = {}

@@ -2,10 +2,20 @@
 // Eq.4: C = sum w_i c_i, D = sum w_i t_i; Eq.5 (:96-99): w_i = T_i alpha_i with
 // alpha_i = 1 - exp(-sigma_i delta_i); readings E (delta_i = the sample's stratum) and G (running
 // product, stop after the first sample with T < tau, black background, depth not normalised).
+#include <cuda_fp16.h>
+
 #include "kernels.h"
 
 namespace r360 {
 
+__device__ __forceinline__ float4 unpack_half4(uint2 q) {
+  const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&q.x));
+  const float2 c = __half22float2(*reinterpret_cast<const __half2*>(&q.y));
+  return make_float4(a.x, a.y, c.x, c.y);
+}
+
+// HALF: the tensor path writes a sample as four binary16 values (sigma, r, g, b), 8 bytes
+template <bool HALF>
 __global__ void __launch_bounds__(128)
 k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __restrict__ out_rgb,
             float* __restrict__ out_depth, PassParams pp) {
@@ -26,14 +36,34 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __res
     for (unsigned s = 0; s < cnt && !done; ++s) {
       const float t_in = b.seg_tin[off + s];
       const float dt = b.seg_dt[off + s];
-      const float4* o = b.out + (size_t)(off + s) * K;
-      // the K samples of a segment are K consecutive float4: fetch them eight at a time, back to back,
-      // so that every 128-byte line is requested once, whole, and not re-fetched after an L1 eviction
+      const size_t o0 = (size_t)(off + s) * K;
+      // the K samples of a segment are K consecutive float4 (uint2 on the tensor path): fetch them eight at a
+      // time, back to back, so that every 128-byte line is requested once, whole, and not re-fetched after an
+      // L1 eviction
       for (int j0 = 0; j0 < K && !done; j0 += 8) {
         float4 v[8];
+        if constexpr (HALF) {
+          const uint2* o = reinterpret_cast<const uint2*>(b.out) + o0;
+          if (j0 + 8 <= K && ((o0 + j0) & 1) == 0) {
+            uint4 q[4];
 #pragma unroll
-        for (int u = 0; u < 8; ++u)
-          if (j0 + u < K) v[u] = __ldcs(o + j0 + u);
+            for (int u = 0; u < 4; ++u) q[u] = __ldcs(reinterpret_cast<const uint4*>(o + j0) + u);
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              v[2 * u] = unpack_half4(make_uint2(q[u].x, q[u].y));
+              v[2 * u + 1] = unpack_half4(make_uint2(q[u].z, q[u].w));
+            }
+          } else {
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+              if (j0 + u < K) v[u] = unpack_half4(__ldcs(o + j0 + u));
+          }
+        } else {
+          const float4* o = b.out + o0;
+#pragma unroll
+          for (int u = 0; u < 8; ++u)
+            if (j0 + u < K) v[u] = __ldcs(o + j0 + u);
+        }
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
           if (j0 + u < K && !done) {
@@ -78,8 +108,9 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __res
 }
 
 void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
-                      float* out_rgb, float* out_depth, const PassParams& pp, cudaStream_t s) {
-  k_composite<<<(f.n_rays + 127) / 128, 128, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
+                      float* out_rgb, float* out_depth, const PassParams& pp, bool half_samples, cudaStream_t s) {
+  if (half_samples) k_composite<true><<<(f.n_rays + 127) / 128, 128, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
+  else k_composite<false><<<(f.n_rays + 127) / 128, 128, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
 }
 
 }  // namespace r360

@@ -48,7 +48,8 @@ struct ChunkBuffers {
   float* seg_tin;        // [G] ray-major
   float* seg_dt;         // [G] ray-major
   SegRec* recs;          // [G * kRecWords] binned by subfield (common.cuh: SegRec)
-  float4* out;           // [G*K] (sigma, r, g, b) per sample, ray-major
+  float4* out;           // [G*K] (sigma, r, g, b) per sample, ray-major; the tensor path stores a sample as four
+                         // binary16 values (8 bytes, the same buffer read as uint2)
   // first kHitCap hits of every ray, kept by k_count so that k_emit re-walks only the rays with more
   float2* hit_t;         // [kHitCap][n_rays] (t_in, delta)
   uint16_t* hit_lab;     // [kHitCap][n_rays]
@@ -95,7 +96,7 @@ cudaError_t launch_mlp_tc(const GridParams& g, const FrameParams& f, const Chunk
                           const SubfieldFrame* frames, int n_bins, int segs_per_tile, int n_sms,
                           cudaStream_t s);
 void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
-                      float* out_rgb, float* out_depth, const PassParams& pp, cudaStream_t s);
+                      float* out_rgb, float* out_depth, const PassParams& pp, bool half_samples, cudaStream_t s);
 // debug: expand binned records into ray-major per-sample t and subfield id
 void launch_export_samples(const GridParams& g, const ChunkBuffers& b, int n_bins, unsigned n_segs,
                            float* t, int32_t* subfield, cudaStream_t s);

@@ -277,11 +277,20 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   const float jf = (float)j + 0.5f;
 
   // MMAs of one operand pair: ks K steps, A from TMEM columns a_col.., B blocks of N rows at b_off
-  auto mma_steps = [&](uint32_t d_col, uint32_t a_col, int b_off, int N, uint32_t idesc, auto ks_c) {
+  // The group's weight buffer never moves, so a block's descriptor is the buffer's plus the block's offset in
+  // 16-byte units -- and every offset is a compile-time constant up to the number of trunk layers: two base values
+  // (the buffer, the colour block) live in uniform registers and nothing is loaded or shifted between the group
+  // barrier and the first tcgen05.mma of a layer (that stretch is on the critical path of every layer).
+  constexpr uint32_t kT1 = (S::KP1 / 16) * S::blk(WD) / 16, kTS = (S::KH / 16) * S::blk(WD) / 16;   // trunk[1], stride
+  constexpr uint32_t kRgb = (S::KC / 16) * S::blk(WD) / 16, kDens = kRgb + (WD / 16) * S::blk(S::NHEAD) / 16;
+  const uint64_t desc0 = smem_desc(sw_addr, 128, 256);
+  const uint32_t desc_hi = (uint32_t)(desc0 >> 32);
+  const uint32_t dl0 = (uint32_t)desc0, dlc = dl0 + kT1 + (uint32_t)(net.Hd - 1) * kTS;
+  auto mma_steps = [&](uint32_t d_col, uint32_t a_col, uint32_t lo, int N, uint32_t idesc, auto ks_c) {
     constexpr int ks = decltype(ks_c)::value;
 #pragma unroll
     for (int s = 0; s < ks; ++s)
-      mma_ts(d_col, a_col + 8 * s, smem_desc(sw_addr + b_off + s * S::blk(N), 128, 256), idesc, s > 0);
+      mma_ts(d_col, a_col + 8 * s, ((uint64_t)desc_hi << 32) | (lo + (uint32_t)(s * (S::blk(N) >> 4))), idesc, s > 0);
   };
   // publish this thread's A row to the group's issuing thread
   auto publish = [&]() {
@@ -385,7 +394,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     if (warp == 0) {
       if (elect_one()) {
         fence_after_sync();
-        mma_steps(mD, mA, lay.trunk[0], WD, idesc_w, std::integral_constant<int, S::KP1 / 16>{});
+        mma_steps(mD, mA, dl0, WD, idesc_w, std::integral_constant<int, S::KP1 / 16>{});
         mma_commit(bar_d);
       }
       __syncwarp();
@@ -409,7 +418,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
       if (warp == 0) {
         if (elect_one()) {
           fence_after_sync();
-          mma_steps(mD, mA, lay.trunk[l], WD, idesc_w, std::integral_constant<int, S::KH / 16>{});
+          mma_steps(mD, mA, dl0 + kT1 + (uint32_t)(l - 1) * kTS, WD, idesc_w, std::integral_constant<int, S::KH / 16>{});
           mma_commit(bar_d);
         }
         __syncwarp();
@@ -422,7 +431,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     if (warp == 0) {
       if (elect_one()) {
         fence_after_sync();
-        mma_steps(mD, mA, lay.col, WD, idesc_w, std::integral_constant<int, S::KC / 16>{});
+        mma_steps(mD, mA, dlc, WD, idesc_w, std::integral_constant<int, S::KC / 16>{});
         mma_commit(bar_d);
       }
       __syncwarp();
@@ -438,8 +447,8 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     if (warp == 0) {
       if (elect_one()) {
         fence_after_sync();
-        mma_steps(mD, mA + S::A_FD, lay.rgb, S::NHEAD, idesc_h, std::integral_constant<int, WD / 16>{});
-        mma_steps(mD + S::NHEAD, mA + S::A_H, lay.dens, S::NHEAD, idesc_h, std::integral_constant<int, WD / 16>{});
+        mma_steps(mD, mA + S::A_FD, dlc + kRgb, S::NHEAD, idesc_h, std::integral_constant<int, WD / 16>{});
+        mma_steps(mD + S::NHEAD, mA + S::A_H, dlc + kDens, S::NHEAD, idesc_h, std::integral_constant<int, WD / 16>{});
         mma_commit(bar_d);
       }
       __syncwarp();
@@ -452,12 +461,12 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     wait_ld();
     // ---- activations (A4), fp32
     const float sigma_raw = __uint_as_float(sraw[0]) + hb.w;
-    float4 o4;
-    o4.x = net.act == 1 ? fast_softplus(sigma_raw) : fmaxf(sigma_raw, 0.0f);
-    o4.y = fast_sigmoid(__uint_as_float(craw[0]) + hb.x);
-    o4.z = fast_sigmoid(__uint_as_float(craw[1]) + hb.y);
-    o4.w = fast_sigmoid(__uint_as_float(craw[2]) + hb.z);
-    if (active) b.out[(size_t)rec.w * K + j] = o4;
+    // a sample leaves as four binary16 values (sigma clamped to the largest finite one): 8 bytes
+    const float sigma = fminf(net.act == 1 ? fast_softplus(sigma_raw) : fmaxf(sigma_raw, 0.0f), 65504.0f);
+    uint2 o2;
+    o2.x = pack_f16(sigma, fast_sigmoid(__uint_as_float(craw[0]) + hb.x));
+    o2.y = pack_f16(fast_sigmoid(__uint_as_float(craw[1]) + hb.y), fast_sigmoid(__uint_as_float(craw[2]) + hb.z));
+    if (active) reinterpret_cast<uint2*>(b.out)[(size_t)rec.w * K + j] = o2;
   }
   fence_before_sync();
   __syncthreads();

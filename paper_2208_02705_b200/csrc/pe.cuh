@@ -22,6 +22,12 @@ __device__ __forceinline__ uint32_t pack_bf16_relu(float lo, float hi) {
   asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
   return r;
 }
+// two fp32 -> packed binary16 x2 (lo in the lower half), round to nearest even
+__device__ __forceinline__ uint32_t pack_f16(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
 
 // sin and cos on |x| <= 1 (normalised positions, reading A3, and unit direction components) by
 // their Taylor polynomials (remainders x^13/13! and x^14/14! are below binary32 resolution).

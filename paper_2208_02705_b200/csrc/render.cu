@@ -206,7 +206,7 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
         launches += 1;
       }
       if (pev) cudaEventRecord(pev->e[4], s);
-      launch_composite(sc->grid_p, f, sc->buf, sc->desc.t_threshold, out_rgb, out_depth, pp, s);
+      launch_composite(sc->grid_p, f, sc->buf, sc->desc.t_threshold, out_rgb, out_depth, pp, sc->precision == 1, s);
       launches += 1;
       R360_CUDA(cudaGetLastError());
       if (pev) cudaEventRecord(pev->e[5], s);
