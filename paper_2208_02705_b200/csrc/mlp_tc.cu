@@ -299,6 +299,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     group_sync_r(bar_id);
   };
   auto wait_acc = [&]() {
+    asm volatile("" : "+r"(par_d));          // in a vector register: nothing is moved inside the spin loop
     mbar_wait(bar_d, par_d);
     par_d ^= 1;
     fence_after_sync();
@@ -412,13 +413,15 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     wait_acc();
     tmem_st_x16(tA + S::A_FD, ad);                           // parks behind h for every later layer
     // ---- trunk-2..Hd: A = [h, 1, 1, ...]
-    for (int l = 1; l < net.Hd; ++l) {
+    // (the loop runs on the descriptor itself: its end value is already in a uniform register, a comparison with
+    // net.Hd would put a parameter load between the accumulator wait and the tcgen05.ld of the next layer)
+    for (uint32_t dlt = dl0 + kT1; dlt != dlc; dlt += kTS) {
       d_to_a(tA + S::A_H);
       publish();
       if (warp == 0) {
         if (elect_one()) {
           fence_after_sync();
-          mma_steps(mD, mA, dl0 + kT1 + (uint32_t)(l - 1) * kTS, WD, idesc_w, std::integral_constant<int, S::KH / 16>{});
+          mma_steps(mD, mA, dlt, WD, idesc_w, std::integral_constant<int, S::KH / 16>{});
           mma_commit(bar_d);
         }
         __syncwarp();

@@ -38,9 +38,19 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
+// the spin loop is one asm block so that its body is try_wait + branch only (written as a C loop, ptxas moves the
+// parity operand into a register again in every iteration: one more issue slot per spin)
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  while (!mbar_try_wait(bar, parity)) {
-  }
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "R360_WAIT:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra R360_DONE;\n\t"
+      "bra R360_WAIT;\n\t"
+      "R360_DONE:\n\t}"
+      :
+      : "r"(smem_u32(bar)), "r"(parity)
+      : "memory");
 }
 
 // ---- named barrier over one 128-thread tile group (id 1..15; id 0 is __syncthreads) -----------
