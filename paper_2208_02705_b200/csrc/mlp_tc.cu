@@ -190,8 +190,15 @@ __device__ __forceinline__ float fast_softplus(float x) {
 // recurrence and stored K step by K step (16 values = 8 TMEM columns), so that few values are live.
 __device__ __forceinline__ void store_pe_row(uint32_t tA, const float q[3]) {
   float s[3], c[3];
-#pragma unroll
-  for (int a = 0; a < 3; ++a) sincos_unit(q[a], s[a], c[a]);
+  uint64_t S2, C2;
+  sincos_unit2(pack_f32x2(q[0], q[1]), S2, C2);
+  unpack_f32x2(S2, s[0], s[1]);
+  unpack_f32x2(C2, c[0], c[1]);
+  sincos_unit(q[2], s[2], c[2]);
+  // x and y advance together in packed binary32 pairs (add/mul/fma.f32x2: one issue slot for two lanes of the
+  // FMA pipe, which this kernel leaves three quarters idle while it is short of issue slots); z stays scalar.
+  // Double angle as s' = (2c) s, c' = (2c) c - 1: no negated operand, which the packed forms do not have.
+  const uint64_t M1 = pack_f32x2(-1.0f, -1.0f), M01 = pack_f32x2(0.0f, -1.0f);
   float buf[16];
 #pragma unroll
   for (int idx = 0; idx < 64; ++idx) {
@@ -202,14 +209,14 @@ __device__ __forceinline__ void store_pe_row(uint32_t tA, const float q[3]) {
       v = 1.0f;                                   // meets the bias row of B
     } else {
       const int l = (idx - 3) / 6, r = (idx - 3) % 6;
-      if (r == 0 && l > 0) {                      // next level: s' = 2 s c, c' = 1 - 2 s^2
-#pragma unroll
-        for (int a = 0; a < 3; ++a) {
-          const float t = s[a] + s[a];
-          const float s2 = t * c[a];
-          c[a] = fmaf(-t, s[a], 1.0f);
-          s[a] = s2;
-        }
+      if (r == 0 && l > 0) {                      // next level
+        const uint64_t Q = add_f32x2(C2, C2);
+        S2 = mul_f32x2(Q, S2);
+        C2 = fma_f32x2(Q, C2, M1);
+        unpack_f32x2(S2, s[0], s[1]);
+        unpack_f32x2(C2, c[0], c[1]);
+        const float t = c[2] + c[2];              // z: (s, c) as one pair, (s', c') = t (s, c) + (0, -1)
+        unpack_f32x2(fma_f32x2(pack_f32x2(t, t), pack_f32x2(s[2], c[2]), M01), s[2], c[2]);
       }
       v = r < 3 ? s[r] : c[r - 3];
     }

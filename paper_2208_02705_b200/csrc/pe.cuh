@@ -29,6 +29,31 @@ __device__ __forceinline__ uint32_t pack_f16(float lo, float hi) {
   return r;
 }
 
+// packed binary32 pairs (sm_100: add / mul / fma .f32x2 on a 64-bit register pair)
+__device__ __forceinline__ uint64_t pack_f32x2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void unpack_f32x2(uint64_t v, float& lo, float& hi) {
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ uint64_t add_f32x2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ uint64_t mul_f32x2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ uint64_t fma_f32x2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+
 // sin and cos on |x| <= 1 (normalised positions, reading A3, and unit direction components) by
 // their Taylor polynomials (remainders x^13/13! and x^14/14! are below binary32 resolution).
 __device__ __forceinline__ void sincos_unit(float x, float& s, float& c) {
@@ -44,6 +69,24 @@ __device__ __forceinline__ void sincos_unit(float x, float& s, float& c) {
   pc = fmaf(x2, pc, 4.1666667e-2f);                       // 1/4!
   pc = fmaf(x2, pc, -0.5f);
   c = fmaf(x2, pc, 1.0f);
+}
+
+// the same for two arguments at once in a packed pair
+__device__ __forceinline__ void sincos_unit2(uint64_t x, uint64_t& s, uint64_t& c) {
+#define R360_K2(v) pack_f32x2(v, v)
+  const uint64_t x2 = mul_f32x2(x, x);
+  uint64_t ps = fma_f32x2(x2, R360_K2(-2.5052108e-8f), R360_K2(2.7557319e-6f));
+  ps = fma_f32x2(x2, ps, R360_K2(-1.9841270e-4f));
+  ps = fma_f32x2(x2, ps, R360_K2(8.3333333e-3f));
+  ps = fma_f32x2(x2, ps, R360_K2(-1.6666667e-1f));
+  s = fma_f32x2(mul_f32x2(x, x2), ps, x);
+  uint64_t pc = fma_f32x2(x2, R360_K2(2.0876757e-9f), R360_K2(-2.7557319e-7f));
+  pc = fma_f32x2(x2, pc, R360_K2(2.4801587e-5f));
+  pc = fma_f32x2(x2, pc, R360_K2(-1.3888889e-3f));
+  pc = fma_f32x2(x2, pc, R360_K2(4.1666667e-2f));
+  pc = fma_f32x2(x2, pc, R360_K2(-0.5f));
+  c = fma_f32x2(x2, pc, R360_K2(1.0f));
+#undef R360_K2
 }
 
 // F(x) for L levels from one sincos per component and the double-angle recurrence
