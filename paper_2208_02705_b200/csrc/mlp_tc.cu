@@ -398,6 +398,19 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
 
     // ---- trunk-1: A = [F(q), 1]
     store_pe_row(tA, q);
+    // the ray's direction block [1, 1, F(d), 0 0 0]: requested before the group barrier so that the load runs
+    // behind the barrier, the MMA issue and the MMA itself (asked for after the issue it arrived later than the
+    // accumulators: 4 % of the kernel's stall samples sat on the tcgen05.st below)
+    uint32_t ad[16];
+    {
+      const uint4* db = b.dirblk + (size_t)rec.x * 4;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        uint4 v;
+        asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(db + c));
+        ad[4 * c] = v.x; ad[4 * c + 1] = v.y; ad[4 * c + 2] = v.z; ad[4 * c + 3] = v.w;
+      }
+    }
     publish();
     if (warp == 0) {
       if (elect_one()) {
@@ -406,16 +419,6 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
         mma_commit(bar_d);
       }
       __syncwarp();
-    }
-    // while the tensor core works: fetch the ray's direction block [1, 1, F(d), 0 0 0]
-    uint32_t ad[16];
-    {
-      const uint4* db = b.dirblk + (size_t)rec.x * 4;
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        const uint4 v = __ldg(db + c);
-        ad[4 * c] = v.x; ad[4 * c + 1] = v.y; ad[4 * c + 2] = v.z; ad[4 * c + 3] = v.w;
-      }
     }
     wait_acc();
     tmem_st_x16(tA + S::A_FD, ad);                           // parks behind h for every later layer
