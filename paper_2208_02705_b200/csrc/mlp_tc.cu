@@ -371,12 +371,10 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
         rd = __ldg(rp + 1);                                  // direction, pose
       }
     }
-    // hide DRAM latency without registers: this tile's direction block (read after trunk-1 is issued) goes to
-    // L2 now; the next tile's records (same subfield, so their place is known) travel to shared memory with
+    // hide DRAM latency without registers: the next tile's records (same subfield, so their place is known) travel to shared memory with
     // cp.async and the records of the tile after it go to L2
     const bool stage_next = spt <= kStageSegs && tile + 1 < tile1 && tile + 1 < k_tile_end;
     if (j == 0) {
-      if (active) prefetch_l2(b.dirblk + (size_t)rec.x * 4);
       const unsigned sn = seg0 + spt + sidx;
       if (sn < k_seg_end) {
         if (stage_next) {

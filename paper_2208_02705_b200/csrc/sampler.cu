@@ -318,18 +318,29 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
     }
   }
   bool more = replay ? h < h_end : w.alive;
+  // replay: the next hit is requested one round ahead, so two rounds of loads are in flight per lane
+  float2 td_n = make_float2(0.f, 0.f);
+  uint32_t lab_n = 0;
+  if (replay && h < h_end) {
+    const size_t i = (size_t)h * f.n_rays + r;
+    td_n = b.hit_t[i];
+    lab_n = b.hit_lab[i];
+  }
   while (__any_sync(0xffffffffu, more)) {
     uint32_t lab = 0;
     float t_in = 0.f, dt = 0.f;
     bool hit = false;
     if (replay) {
       if (h < h_end) {
-        const size_t i = (size_t)h * f.n_rays + r;
-        const float2 td = b.hit_t[i];
-        t_in = td.x; dt = td.y;
-        lab = b.hit_lab[i];
+        t_in = td_n.x; dt = td_n.y;
+        lab = lab_n;
         hit = true;
         ++h;
+        if (h < h_end) {
+          const size_t i = (size_t)h * f.n_rays + r;
+          td_n = b.hit_t[i];
+          lab_n = b.hit_lab[i];
+        }
       }
       more = h < h_end;
     } else {
