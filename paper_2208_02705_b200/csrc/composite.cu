@@ -33,7 +33,49 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __res
       T = b.st_T[r];
     }
     bool done = false;
-    for (unsigned s = 0; s < cnt && !done; ++s) {
+    unsigned s_begin = 0;
+    if constexpr (HALF) {
+      if (K == 8 && cnt) {
+        // the common tensor-path case (8 samples = 64 bytes per segment): the NEXT segment's samples are requested
+        // before this one's are composited, so two segments (a whole 128-byte line) are in flight per ray
+        const uint4* o = reinterpret_cast<const uint4*>(reinterpret_cast<const uint2*>(b.out) + (size_t)off * 8);
+        uint4 q[4], qn[4];
+        float t_in = b.seg_tin[off], dt = b.seg_dt[off], t_in_n = 0.f, dt_n = 0.f;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) q[u] = __ldcs(o + u);
+        for (unsigned s = 0; s < cnt && !done; ++s) {
+          if (s + 1 < cnt) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) qn[u] = __ldcs(o + (size_t)(s + 1) * 4 + u);
+            t_in_n = b.seg_tin[off + s + 1];
+            dt_n = b.seg_dt[off + s + 1];
+          }
+#pragma unroll
+          for (int u = 0; u < 8; ++u) {
+            if (!done) {
+              const uint4 qq = q[u >> 1];
+              const float4 v = unpack_half4((u & 1) ? make_uint2(qq.z, qq.w) : make_uint2(qq.x, qq.y));
+              const float t = __fmaf_rn((float)u + 0.5f, dt, t_in);
+              const float alpha = 1.0f - expf(-v.x * dt);
+              const float w = T * alpha;
+              C0 = fmaf(w, v.y, C0);
+              C1 = fmaf(w, v.z, C1);
+              C2 = fmaf(w, v.w, C2);
+              D = fmaf(w, t, D);
+              T = T * (1.0f - alpha);
+              ++used;
+              if (T < tau) done = true;
+            }
+          }
+#pragma unroll
+          for (int u = 0; u < 4; ++u) q[u] = qn[u];
+          t_in = t_in_n;
+          dt = dt_n;
+        }
+        s_begin = cnt;                     // nothing left for the general loop
+      }
+    }
+    for (unsigned s = s_begin; s < cnt && !done; ++s) {
       const float t_in = b.seg_tin[off + s];
       const float dt = b.seg_dt[off + s];
       const size_t o0 = (size_t)(off + s) * K;
