@@ -75,6 +75,8 @@ def test_render_bf16_config2(r360, oracle, scene2):
 
 
 @pytest.mark.parametrize("over", [dict(samples_per_voxel=12), dict(samples_per_voxel=5),
+                                  dict(samples_per_voxel=1), dict(samples_per_voxel=16),
+                                  dict(samples_per_voxel=128),
                                   dict(density_activation=0), dict(t_threshold=0.0)])
 def test_render_bf16_variants(r360, oracle, scene1, over):
     _cmp(r360, oracle, scene1, **over)
@@ -107,6 +109,15 @@ def test_render_bf16_early_out(r360, oracle, scene1):
     e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 40.0), amb_band=0.2,
                              tol=4e-3)
     print("dense stress bf16 max rgb err", e_rgb)
+
+
+@pytest.mark.parametrize("act", [0, 1])
+def test_render_bf16_saturating_density(r360, oracle, scene1, act):
+    # density far beyond binary16's range: the tensor path stores sigma as binary16 clamped to 65504, alpha is 1
+    # either way, so every pixel is the colour of its first sample (per-sample bf16 error: the 4e-3 bound above)
+    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 1.0e6), amb_band=0.2,
+                             tol=4e-3, density_activation=act)
+    print("saturating density bf16 max rgb err", e_rgb)
 
 
 def test_bf16_refused_for_other_pe_sizes(r360, scene1):
