@@ -164,6 +164,8 @@ void r360_scene_destroy(r360_scene* sc) {
   cudaFree(sc->d_pass_cnt); cudaFree(sc->buf.pass_off); cudaFree(sc->buf.st_c); cudaFree(sc->buf.st_T);
   cudaFree(sc->d_stage_rgb); cudaFree(sc->d_stage_depth);
   if (sc->h_totals) cudaFreeHost(sc->h_totals);
+  if (sc->copy_stream) cudaStreamDestroy(sc->copy_stream);
+  if (sc->ev_chunk_done) cudaEventDestroy(sc->ev_chunk_done);
   for (auto& ce : sc->events)
     for (auto& e : ce.e) cudaEventDestroy(e);
   cudaGetLastError();

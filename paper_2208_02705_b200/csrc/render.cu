@@ -156,8 +156,10 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
 
 }  // namespace
 
+// host_rgb / host_depth (both or neither): every chunk's part of the image is copied to host memory on a second
+// stream as soon as the chunk is composited, behind the next chunk's kernels (r360_render_batch_host)
 static r360_status render_device(r360_scene* sc, const float* poses, int B, int W, int H, float* out_rgb,
-                                 float* out_depth) {
+                                 float* out_depth, float* host_rgb = nullptr, float* host_depth = nullptr) {
   if (!sc || !poses || !out_rgb || !out_depth || B < 1 || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
   if ((long long)W * H >= (1ll << 30)) return R360_ERR_INVALID_ARG;
   const long long total_rays = (long long)B * W * H;
@@ -213,6 +215,14 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
       stats.segments += n_segs;
       stats.mlp_tiles += n_tiles;
     }
+    if (host_rgb) {
+      R360_CUDA(cudaEventRecord(sc->ev_chunk_done, s));
+      R360_CUDA(cudaStreamWaitEvent(sc->copy_stream, sc->ev_chunk_done, 0));
+      R360_CUDA(cudaMemcpyAsync(host_rgb + (size_t)ray0 * 3, out_rgb + (size_t)ray0 * 3, (size_t)n_rays * 3 * sizeof(float),
+                                cudaMemcpyDeviceToHost, sc->copy_stream));
+      R360_CUDA(cudaMemcpyAsync(host_depth + (size_t)ray0, out_depth + (size_t)ray0, (size_t)n_rays * sizeof(float),
+                                cudaMemcpyDeviceToHost, sc->copy_stream));
+    }
   }
   // wavefront: `segments` counts what reached the MLP; the geometric total comes from the walk
   stats.samples_emitted = (sc->wavefront ? (uint64_t)sc->h_totals[3] : stats.segments) * (uint64_t)sc->grid_p.K;
@@ -246,11 +256,16 @@ r360_status r360_render_batch_host(r360_scene* sc, const float* poses, int32_t B
     R360_CUDA(cudaMalloc(&sc->d_stage_depth, R * sizeof(float)));
     sc->stage_rays_cap = R;
   }
-  r360_status st = render_device(sc, poses, B, W, H, sc->d_stage_rgb, sc->d_stage_depth);
+  if (!sc->copy_stream) {
+    R360_CUDA(cudaStreamCreateWithFlags(&sc->copy_stream, cudaStreamNonBlocking));
+    R360_CUDA(cudaEventCreateWithFlags(&sc->ev_chunk_done, cudaEventDisableTiming));
+  }
+  r360_status st = render_device(sc, poses, B, W, H, sc->d_stage_rgb, sc->d_stage_depth, out_rgb_host, out_depth_host);
+  // on an error too: no copy may still be writing the caller's buffers when this returns
+  cudaError_t e1 = cudaStreamSynchronize(sc->copy_stream), e2 = cudaStreamSynchronize(sc->stream);
   if (st != R360_OK) return st;
-  R360_CUDA(cudaMemcpyAsync(out_rgb_host, sc->d_stage_rgb, R * 3 * sizeof(float), cudaMemcpyDeviceToHost, sc->stream));
-  R360_CUDA(cudaMemcpyAsync(out_depth_host, sc->d_stage_depth, R * sizeof(float), cudaMemcpyDeviceToHost, sc->stream));
-  R360_CUDA(cudaStreamSynchronize(sc->stream));
+  if (e1 != cudaSuccess) return r360_cuda_fail(e1, "cudaStreamSynchronize(copy_stream)");
+  if (e2 != cudaSuccess) return r360_cuda_fail(e2, "cudaStreamSynchronize(stream)");
   return R360_OK;
 }
 

@@ -38,6 +38,8 @@ struct r360_scene {
   float* d_stage_rgb = nullptr;
   float* d_stage_depth = nullptr;
   size_t stage_rays_cap = 0;
+  cudaStream_t copy_stream = nullptr;       // chunk k's image part goes to the host behind chunk k+1's kernels
+  cudaEvent_t ev_chunk_done = nullptr;
   // configuration
   cudaStream_t stream = nullptr;
   int precision = 0;

@@ -152,6 +152,10 @@ def test_chunked_and_batched_equal_single(r360, scene1):
     assert torch.equal(rgbb[0], rgb0) and torch.equal(rgbb[1], rgb2) and torch.equal(db[1], d2)
     h_rgb, h_d = gpu.render_batch_host(poses, 64, 32)
     assert np.array_equal(h_rgb, rgbb.cpu().numpy()) and np.array_equal(h_d, db.cpu().numpy())
+    gpu.set_chunk_rays(300)                                     # 14 chunks, each copied to the host behind the next
+    h_rgb2, h_d2 = gpu.render_batch_host(poses, 64, 32)
+    assert gpu.stats().chunks == 14
+    assert np.array_equal(h_rgb2, h_rgb) and np.array_equal(h_d2, h_d)
 
 
 def test_render_rejects_bad_arguments(r360, scene1):
