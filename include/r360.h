@@ -93,7 +93,9 @@ r360_status r360_render_batch(r360_scene* scene, const float* poses, int32_t B, 
                               float* out_rgb, float* out_depth);
 
 /* End-to-end convenience: like r360_render_batch but the outputs are HOST buffers
- * (float[B*H*W*3], float[B*H*W]); the call copies device -> host and returns when done. */
+ * (float[B*H*W*3], float[B*H*W]; pinned memory for full PCIe speed); every chunk of rays
+ * (r360_set_chunk_rays) is copied device -> host on a second stream while the next chunk is
+ * rendered; the call returns when all copies are done, also after an error. */
 r360_status r360_render_batch_host(r360_scene* scene, const float* poses, int32_t B, int32_t W, int32_t H,
                                    float* out_rgb_host, float* out_depth_host);
 
