@@ -374,11 +374,14 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     // hide DRAM latency without registers: the next tile's records (same subfield, so their place is known) travel to shared memory with
     // cp.async and the records of the tile after it go to L2
     const bool stage_next = spt <= kStageSegs && tile + 1 < tile1 && tile + 1 < k_tile_end;
-    if (j == 0) {
-      const unsigned sn = seg0 + spt + sidx;
+    // one warp (not the one that issues the MMAs) does this for the whole tile: thread i of warp 3 takes segment i
+    // (K >= 4: at most 32 segments per tile); the other three warps skip the block as a whole
+    const int si = spt <= 32 ? tid - 96 : (j == 0 ? sidx : -1);
+    if (si >= 0 && si < spt) {
+      const unsigned sn = seg0 + spt + si;
       if (sn < k_seg_end) {
         if (stage_next) {
-          uint4* dp = &rec_stage_s[grp][stage_buf ^ 1][sidx * kRecWords];
+          uint4* dp = &rec_stage_s[grp][stage_buf ^ 1][si * kRecWords];
           cp_async_16(dp, b.recs + (size_t)sn * kRecWords);
           cp_async_16(dp + 1, b.recs + (size_t)sn * kRecWords + 1);
         }
