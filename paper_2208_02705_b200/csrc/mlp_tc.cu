@@ -111,7 +111,8 @@ void pack_subfield_t(const NetShape& net, const float* src, void* dstv) {
     uint16_t* d = (uint16_t*)(dst + L.trunk[0]);
     const float* W = s; const float* b = s + WD * kPeP;
     for (int n = 0; n < WD; ++n) {
-      for (int k = 0; k < kPeP; ++k) put(d, WD, n, k, W[n * kPeP + k]);
+      // cosine columns (k = 3 + 6 l + 3 + a) are halved: the kernel's A row holds 2 cos (store_pe_row)
+      for (int k = 0; k < kPeP; ++k) put(d, WD, n, k, (k >= 3 && (k - 3) % 6 >= 3) ? 0.5f * W[n * kPeP + k] : W[n * kPeP + k]);
       put(d, WD, n, kPeP, b[n]);
     }
     s += WD * kPeP + WD;
@@ -189,16 +190,18 @@ __device__ __forceinline__ float fast_softplus(float x) {
 // trunk-1 A row: [F(q) (63), 1] as 32 bf16x2 words, generated level by level with the double-angle
 // recurrence and stored K step by K step (16 values = 8 TMEM columns), so that few values are live.
 __device__ __forceinline__ void store_pe_row(uint32_t tA, const float q[3]) {
-  float s[3], c[3];
-  uint64_t S2, C2;
-  sincos_unit2(pack_f32x2(q[0], q[1]), S2, C2);
+  // The row holds sin and TWICE the cosine of every level (the host halves the matching weight columns, which is
+  // exact in bf16), because the double-angle step on (s, g = 2c) is s' = g s, g' = g g - 2: two operations per
+  // level.  x and y advance together in packed binary32 pairs (add/mul/fma.f32x2: one issue slot for two lanes of
+  // the FMA pipe, which this kernel leaves three quarters idle while it is short of issue slots); z is the pair
+  // (s, g) with (s', g') = g (s, g) + (0, -2): one operation per level.
+  float s[3], c[3];                               // c = 2 cos
+  uint64_t S2, G2;
+  sin_2cos_unit2(pack_f32x2(q[0], q[1]), S2, G2);
   unpack_f32x2(S2, s[0], s[1]);
-  unpack_f32x2(C2, c[0], c[1]);
-  sincos_unit(q[2], s[2], c[2]);
-  // x and y advance together in packed binary32 pairs (add/mul/fma.f32x2: one issue slot for two lanes of the
-  // FMA pipe, which this kernel leaves three quarters idle while it is short of issue slots); z stays scalar.
-  // Double angle as s' = (2c) s, c' = (2c) c - 1: no negated operand, which the packed forms do not have.
-  const uint64_t M1 = pack_f32x2(-1.0f, -1.0f), M01 = pack_f32x2(0.0f, -1.0f);
+  unpack_f32x2(G2, c[0], c[1]);
+  sin_2cos_unit(q[2], s[2], c[2]);
+  const uint64_t M2 = pack_f32x2(-2.0f, -2.0f), M02 = pack_f32x2(0.0f, -2.0f);
   float buf[16];
 #pragma unroll
   for (int idx = 0; idx < 64; ++idx) {
@@ -210,13 +213,11 @@ __device__ __forceinline__ void store_pe_row(uint32_t tA, const float q[3]) {
     } else {
       const int l = (idx - 3) / 6, r = (idx - 3) % 6;
       if (r == 0 && l > 0) {                      // next level
-        const uint64_t Q = add_f32x2(C2, C2);
-        S2 = mul_f32x2(Q, S2);
-        C2 = fma_f32x2(Q, C2, M1);
+        S2 = mul_f32x2(G2, S2);
+        G2 = fma_f32x2(G2, G2, M2);
         unpack_f32x2(S2, s[0], s[1]);
-        unpack_f32x2(C2, c[0], c[1]);
-        const float t = c[2] + c[2];              // z: (s, c) as one pair, (s', c') = t (s, c) + (0, -1)
-        unpack_f32x2(fma_f32x2(pack_f32x2(t, t), pack_f32x2(s[2], c[2]), M01), s[2], c[2]);
+        unpack_f32x2(G2, c[0], c[1]);
+        unpack_f32x2(fma_f32x2(pack_f32x2(c[2], c[2]), pack_f32x2(s[2], c[2]), M02), s[2], c[2]);
       }
       v = r < 3 ? s[r] : c[r - 3];
     }

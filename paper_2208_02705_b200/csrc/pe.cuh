@@ -71,7 +71,40 @@ __device__ __forceinline__ void sincos_unit(float x, float& s, float& c) {
   c = fmaf(x2, pc, 1.0f);
 }
 
+// sin and TWICE the cosine (all cosine coefficients doubled: exact), for the tensor path's recurrence on q = 2 cos
+__device__ __forceinline__ void sin_2cos_unit(float x, float& s, float& q) {
+  const float x2 = x * x;
+  float ps = fmaf(x2, -2.5052108e-8f, 2.7557319e-6f);
+  ps = fmaf(x2, ps, -1.9841270e-4f);
+  ps = fmaf(x2, ps, 8.3333333e-3f);
+  ps = fmaf(x2, ps, -1.6666667e-1f);
+  s = fmaf(x * x2, ps, x);
+  float pc = fmaf(x2, 2.0f * 2.0876757e-9f, 2.0f * -2.7557319e-7f);
+  pc = fmaf(x2, pc, 2.0f * 2.4801587e-5f);
+  pc = fmaf(x2, pc, 2.0f * -1.3888889e-3f);
+  pc = fmaf(x2, pc, 2.0f * 4.1666667e-2f);
+  pc = fmaf(x2, pc, -1.0f);
+  q = fmaf(x2, pc, 2.0f);
+}
 // the same for two arguments at once in a packed pair
+__device__ __forceinline__ void sin_2cos_unit2(uint64_t x, uint64_t& s, uint64_t& q) {
+#define R360_K2(v) pack_f32x2(v, v)
+  const uint64_t x2 = mul_f32x2(x, x);
+  uint64_t ps = fma_f32x2(x2, R360_K2(-2.5052108e-8f), R360_K2(2.7557319e-6f));
+  ps = fma_f32x2(x2, ps, R360_K2(-1.9841270e-4f));
+  ps = fma_f32x2(x2, ps, R360_K2(8.3333333e-3f));
+  ps = fma_f32x2(x2, ps, R360_K2(-1.6666667e-1f));
+  s = fma_f32x2(mul_f32x2(x, x2), ps, x);
+  uint64_t pc = fma_f32x2(x2, R360_K2(2.0f * 2.0876757e-9f), R360_K2(2.0f * -2.7557319e-7f));
+  pc = fma_f32x2(x2, pc, R360_K2(2.0f * 2.4801587e-5f));
+  pc = fma_f32x2(x2, pc, R360_K2(2.0f * -1.3888889e-3f));
+  pc = fma_f32x2(x2, pc, R360_K2(2.0f * 4.1666667e-2f));
+  pc = fma_f32x2(x2, pc, R360_K2(-1.0f));
+  q = fma_f32x2(x2, pc, R360_K2(2.0f));
+#undef R360_K2
+}
+
+// sin and cos of two arguments at once in a packed pair
 __device__ __forceinline__ void sincos_unit2(uint64_t x, uint64_t& s, uint64_t& c) {
 #define R360_K2(v) pack_f32x2(v, v)
   const uint64_t x2 = mul_f32x2(x, x);
