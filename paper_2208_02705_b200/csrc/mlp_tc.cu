@@ -150,11 +150,12 @@ void pack_subfield_t(const NetShape& net, const float* src, void* dstv) {
     }
   }
   {
+    // both heads are ONE operand with K = 2 WD against A = [h | colour activation]: row 3 = density (reads h),
+    // rows 0-2 = rgb (read the colour activation); L.dens is the second half of the same block
     uint16_t* d = (uint16_t*)(dst + L.rgb);
+    for (int k = 0; k < WD; ++k) put(d, S::NHEAD, 3, k, dens[k]);
     for (int n = 0; n < 3; ++n)
-      for (int k = 0; k < WD; ++k) put(d, S::NHEAD, n, k, rgb[n * WD + k]);
-    uint16_t* e = (uint16_t*)(dst + L.dens);
-    for (int k = 0; k < WD; ++k) put(e, S::NHEAD, 0, k, dens[k]);
+      for (int k = 0; k < WD; ++k) put(d, S::NHEAD, n, WD + k, rgb[n * WD + k]);
     float hb[4] = {rgb[3 * WD + 0], rgb[3 * WD + 1], rgb[3 * WD + 2], dens[WD]};
     std::memcpy(dst + L.head_bias, hb, sizeof(hb));
   }
@@ -290,7 +291,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   // (the buffer, the colour block) live in uniform registers and nothing is loaded or shifted between the group
   // barrier and the first tcgen05.mma of a layer (that stretch is on the critical path of every layer).
   constexpr uint32_t kT1 = (S::KP1 / 16) * S::blk(WD) / 16, kTS = (S::KH / 16) * S::blk(WD) / 16;   // trunk[1], stride
-  constexpr uint32_t kRgb = (S::KC / 16) * S::blk(WD) / 16, kDens = kRgb + (WD / 16) * S::blk(S::NHEAD) / 16;
+  constexpr uint32_t kRgb = (S::KC / 16) * S::blk(WD) / 16;                                         // heads
   const uint64_t desc0 = smem_desc(sw_addr, 128, 256);
   const uint32_t desc_hi = (uint32_t)(desc0 >> 32);
   const uint32_t dl0 = (uint32_t)desc0, dlc = dl0 + kT1 + (uint32_t)(net.Hd - 1) * kTS;
@@ -452,8 +453,8 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
       __syncwarp();
     }
     wait_acc();
-    // ---- heads: rgb from the colour activation (takes the direction block's columns), density
-    //      from h (still in place); both N = 16, accumulators side by side
+    // ---- heads: one N = 16 operand over A = [h | colour activation] (the activation takes the direction block's
+    //      columns, h is still in place): outputs r, g, b, sigma in four adjacent accumulator columns
     d_to_a(tA + S::A_FD);
     cp_async_wait_all();                                     // the staged records are complete before this barrier
     publish();
@@ -462,20 +463,18 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     if (warp == 0) {
       if (elect_one()) {
         fence_after_sync();
-        mma_steps(mD, mA + S::A_FD, dlc + kRgb, S::NHEAD, idesc_h, std::integral_constant<int, WD / 16>{});
-        mma_steps(mD + S::NHEAD, mA + S::A_H, dlc + kDens, S::NHEAD, idesc_h, std::integral_constant<int, WD / 16>{});
+        mma_steps(mD, mA + S::A_H, dlc + kRgb, S::NHEAD, idesc_h, std::integral_constant<int, 2 * WD / 16>{});
         mma_commit(bar_d);
       }
       __syncwarp();
     }
     const float4 hb = *reinterpret_cast<const float4*>(sw + lay.head_bias);
     wait_acc();
-    uint32_t craw[4], sraw[4];
+    uint32_t craw[4];                                        // r, g, b, sigma
     tmem_ld_x4(tD, craw);
-    tmem_ld_x4(tD + S::NHEAD, sraw);
     wait_ld();
     // ---- activations (A4), fp32
-    const float sigma_raw = __uint_as_float(sraw[0]) + hb.w;
+    const float sigma_raw = __uint_as_float(craw[3]) + hb.w;
     // a sample leaves as four binary16 values (sigma clamped to the largest finite one): 8 bytes
     const float sigma = fminf(net.act == 1 ? fast_softplus(sigma_raw) : fmaxf(sigma_raw, 0.0f), 65504.0f);
     uint2 o2;
