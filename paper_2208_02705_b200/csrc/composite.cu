@@ -14,8 +14,53 @@ __device__ __forceinline__ float4 unpack_half4(uint2 q) {
   return make_float4(a.x, a.y, c.x, c.y);
 }
 
+// Tensor path, KK samples of 8 bytes per segment (KK even: whole 16-byte words): the NEXT segment's samples are
+// requested before this one's are composited, so two segments are in flight per ray.
+template <int KK>
+__device__ __forceinline__ void composite_half_segments(const ChunkBuffers& b, unsigned off, unsigned cnt, float tau,
+                                                        float& T, float& C0, float& C1, float& C2, float& D,
+                                                        unsigned& used, bool& done) {
+  constexpr int Q = KK / 2;
+  const uint4* o = reinterpret_cast<const uint4*>(reinterpret_cast<const uint2*>(b.out) + (size_t)off * KK);
+  uint4 q[Q], qn[Q];
+  float t_in = b.seg_tin[off], dt = b.seg_dt[off], t_in_n = 0.f, dt_n = 0.f;
+#pragma unroll
+  for (int u = 0; u < Q; ++u) q[u] = __ldcs(o + u);
+  for (unsigned s = 0; s < cnt && !done; ++s) {
+    if (s + 1 < cnt) {
+#pragma unroll
+      for (int u = 0; u < Q; ++u) qn[u] = __ldcs(o + (size_t)(s + 1) * Q + u);
+      t_in_n = b.seg_tin[off + s + 1];
+      dt_n = b.seg_dt[off + s + 1];
+    }
+#pragma unroll
+    for (int u = 0; u < KK; ++u) {
+      if (!done) {
+        const uint4 qq = q[u >> 1];
+        const float4 v = unpack_half4((u & 1) ? make_uint2(qq.z, qq.w) : make_uint2(qq.x, qq.y));
+        const float t = __fmaf_rn((float)u + 0.5f, dt, t_in);
+        const float alpha = 1.0f - expf(-v.x * dt);
+        const float w = T * alpha;
+        C0 = fmaf(w, v.y, C0);
+        C1 = fmaf(w, v.z, C1);
+        C2 = fmaf(w, v.w, C2);
+        D = fmaf(w, t, D);
+        T = T * (1.0f - alpha);
+        ++used;
+        if (T < tau) done = true;
+      }
+    }
+#pragma unroll
+    for (int u = 0; u < Q; ++u) q[u] = qn[u];
+    t_in = t_in_n;
+    dt = dt_n;
+  }
+}
+
 // HALF: the tensor path writes a sample as four binary16 values (sigma, r, g, b), 8 bytes
-template <bool HALF>
+// KFAST: 8 / 12 / 16 = the tensor path's pipelined loop for that K (its own kernel, so that the wider variants'
+// registers do not cost the K = 8 case occupancy); 0 = the general loop
+template <bool HALF, int KFAST>
 __global__ void __launch_bounds__(128)
 k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __restrict__ out_rgb,
             float* __restrict__ out_depth, PassParams pp) {
@@ -34,46 +79,9 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __res
     }
     bool done = false;
     unsigned s_begin = 0;
-    if constexpr (HALF) {
-      if (K == 8 && cnt) {
-        // the common tensor-path case (8 samples = 64 bytes per segment): the NEXT segment's samples are requested
-        // before this one's are composited, so two segments (a whole 128-byte line) are in flight per ray
-        const uint4* o = reinterpret_cast<const uint4*>(reinterpret_cast<const uint2*>(b.out) + (size_t)off * 8);
-        uint4 q[4], qn[4];
-        float t_in = b.seg_tin[off], dt = b.seg_dt[off], t_in_n = 0.f, dt_n = 0.f;
-#pragma unroll
-        for (int u = 0; u < 4; ++u) q[u] = __ldcs(o + u);
-        for (unsigned s = 0; s < cnt && !done; ++s) {
-          if (s + 1 < cnt) {
-#pragma unroll
-            for (int u = 0; u < 4; ++u) qn[u] = __ldcs(o + (size_t)(s + 1) * 4 + u);
-            t_in_n = b.seg_tin[off + s + 1];
-            dt_n = b.seg_dt[off + s + 1];
-          }
-#pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            if (!done) {
-              const uint4 qq = q[u >> 1];
-              const float4 v = unpack_half4((u & 1) ? make_uint2(qq.z, qq.w) : make_uint2(qq.x, qq.y));
-              const float t = __fmaf_rn((float)u + 0.5f, dt, t_in);
-              const float alpha = 1.0f - expf(-v.x * dt);
-              const float w = T * alpha;
-              C0 = fmaf(w, v.y, C0);
-              C1 = fmaf(w, v.z, C1);
-              C2 = fmaf(w, v.w, C2);
-              D = fmaf(w, t, D);
-              T = T * (1.0f - alpha);
-              ++used;
-              if (T < tau) done = true;
-            }
-          }
-#pragma unroll
-          for (int u = 0; u < 4; ++u) q[u] = qn[u];
-          t_in = t_in_n;
-          dt = dt_n;
-        }
-        s_begin = cnt;                     // nothing left for the general loop
-      }
+    if constexpr (HALF && KFAST > 0) {
+      if (cnt) composite_half_segments<KFAST>(b, off, cnt, tau, T, C0, C1, C2, D, used, done);
+      s_begin = cnt;                       // nothing left for the general loop
     }
     for (unsigned s = s_begin; s < cnt && !done; ++s) {
       const float t_in = b.seg_tin[off + s];
@@ -151,8 +159,12 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __res
 
 void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
                       float* out_rgb, float* out_depth, const PassParams& pp, bool half_samples, cudaStream_t s) {
-  if (half_samples) k_composite<true><<<(f.n_rays + 127) / 128, 128, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
-  else k_composite<false><<<(f.n_rays + 127) / 128, 128, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
+  const dim3 grid((f.n_rays + 127) / 128), block(128);
+  if (!half_samples) k_composite<false, 0><<<grid, block, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
+  else if (g.K == 8) k_composite<true, 8><<<grid, block, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
+  else if (g.K == 12) k_composite<true, 12><<<grid, block, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
+  else if (g.K == 16) k_composite<true, 16><<<grid, block, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
+  else k_composite<true, 0><<<grid, block, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
 }
 
 }  // namespace r360
