@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(CSRC, "libr360.so")
 SOURCES = ["capi.cu", "render.cu", "sampler.cu", "mlp_fp32.cu", "mlp_tc.cu", "composite.cu", "assign.cu", "floorplan.cu", "fuse.cu"]
-HEADERS = ["common.cuh", "kernels.h", "scene.h", os.path.join("..", "..", "include", "r360.h")]
+HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))) + [os.path.join("..", "..", "include", "r360.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall", "--shared", "-cudart", "static"]
 
