@@ -280,6 +280,10 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   const uint32_t sw_addr = smem_u32(sw);
   const uint32_t idesc_w = instr_desc_bf16(128, WD), idesc_h = instr_desc_bf16(128, S::NHEAD);
   const uint32_t bar_id = (uint32_t)grp + 1;
+  // warp w of every group runs on scheduler w.  The warp that issues the MMAs and the one that stages the next
+  // tile's records carry extra instructions, so both roles rotate with the group: each scheduler then hosts the
+  // same number of issuing and staging warps instead of scheduler 0 all issuers and scheduler 3 all stagers
+  const int iss_warp = grp & 3, stg_warp = (grp + 2) & 3;
   uint32_t par_d = 0, par_w = 0;
   const int K = g.K;
   const int sidx = tid / K, j = tid - sidx * K;
@@ -378,7 +382,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     const bool stage_next = spt <= kStageSegs && tile + 1 < tile1 && tile + 1 < k_tile_end;
     // one warp (not the one that issues the MMAs) does this for the whole tile: thread i of warp 3 takes segment i
     // (K >= 4: at most 32 segments per tile); the other three warps skip the block as a whole
-    const int si = spt <= 32 ? tid - 96 : (j == 0 ? sidx : -1);
+    const int si = spt <= 32 ? tid - 32 * stg_warp : (j == 0 ? sidx : -1);
     if (si >= 0 && si < spt) {
       const unsigned sn = seg0 + spt + si;
       if (sn < k_seg_end) {
@@ -415,7 +419,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
       }
     }
     publish();
-    if (warp == 0) {
+    if (warp == iss_warp) {
       if (elect_one()) {
         fence_after_sync();
         mma_steps(mD, mA, dl0, WD, idesc_w, std::integral_constant<int, S::KP1 / 16>{});
@@ -431,7 +435,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     for (uint32_t dlt = dl0 + kT1; dlt != dlc; dlt += kTS) {
       d_to_a(tA + S::A_H);
       publish();
-      if (warp == 0) {
+      if (warp == iss_warp) {
         if (elect_one()) {
           fence_after_sync();
           mma_steps(mD, mA, dlt, WD, idesc_w, std::integral_constant<int, S::KH / 16>{});
@@ -444,7 +448,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     // ---- colour (feature layer folded in): A = [h, 1, 1, F(d), 0 0 0]
     d_to_a(tA + S::A_H);
     publish();
-    if (warp == 0) {
+    if (warp == iss_warp) {
       if (elect_one()) {
         fence_after_sync();
         mma_steps(mD, mA, dlc, WD, idesc_w, std::integral_constant<int, S::KC / 16>{});
@@ -460,7 +464,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     publish();
     staged = stage_next;
     stage_buf ^= 1;
-    if (warp == 0) {
+    if (warp == iss_warp) {
       if (elect_one()) {
         fence_after_sync();
         mma_steps(mD, mA + S::A_H, dlc + kRgb, S::NHEAD, idesc_h, std::integral_constant<int, 2 * WD / 16>{});
