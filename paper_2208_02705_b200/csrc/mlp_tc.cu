@@ -380,21 +380,6 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     // hide DRAM latency without registers: the next tile's records (same subfield, so their place is known) travel to shared memory with
     // cp.async and the records of the tile after it go to L2
     const bool stage_next = spt <= kStageSegs && tile + 1 < tile1 && tile + 1 < k_tile_end;
-    // one warp (not the one that issues the MMAs) does this for the whole tile: thread i of warp 3 takes segment i
-    // (K >= 4: at most 32 segments per tile); the other three warps skip the block as a whole
-    const int si = spt <= 32 ? tid - 32 * stg_warp : (j == 0 ? sidx : -1);
-    if (si >= 0 && si < spt) {
-      const unsigned sn = seg0 + spt + si;
-      if (sn < k_seg_end) {
-        if (stage_next) {
-          uint4* dp = &rec_stage_s[grp][stage_buf ^ 1][si * kRecWords];
-          cp_async_16(dp, b.recs + (size_t)sn * kRecWords);
-          cp_async_16(dp + 1, b.recs + (size_t)sn * kRecWords + 1);
-        }
-        if (sn + spt < k_seg_end) prefetch_l2(b.recs + (size_t)(sn + spt) * kRecWords);
-      }
-    }
-    cp_async_commit();
     const float* P = f.poses + rd.w * 12;
     const float t = __fmaf_rn(jf, __uint_as_float(rec.z), __uint_as_float(rec.y));   // reading D
     float q[3];                                              // reading A3
@@ -427,6 +412,23 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
       }
       __syncwarp();
     }
+    // (behind the first layer's barrier: in front of it the staging warp reached the barrier last and the whole
+    // group waited for it)
+    // one warp (not the one that issues the MMAs) does this for the whole tile: thread i of warp 3 takes segment i
+    // (K >= 4: at most 32 segments per tile); the other three warps skip the block as a whole
+    const int si = spt <= 32 ? tid - 32 * stg_warp : (j == 0 ? sidx : -1);
+    if (si >= 0 && si < spt) {
+      const unsigned sn = seg0 + spt + si;
+      if (sn < k_seg_end) {
+        if (stage_next) {
+          uint4* dp = &rec_stage_s[grp][stage_buf ^ 1][si * kRecWords];
+          cp_async_16(dp, b.recs + (size_t)sn * kRecWords);
+          cp_async_16(dp + 1, b.recs + (size_t)sn * kRecWords + 1);
+        }
+        if (sn + spt < k_seg_end) prefetch_l2(b.recs + (size_t)(sn + spt) * kRecWords);
+      }
+    }
+    cp_async_commit();
     wait_acc();
     tmem_st_x16(tA + S::A_FD, ad);                           // parks behind h for every later layer
     // ---- trunk-2..Hd: A = [h, 1, 1, ...]
