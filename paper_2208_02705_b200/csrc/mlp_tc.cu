@@ -179,13 +179,22 @@ void tc_pack_subfield(const NetShape& net, const float* src_blob, void* dst) {
 using namespace tc;
 
 // heads of the bf16 path: ex2/lg2/rcp approximations (relative error ~2^-22, far below bf16)
+// exp2 / log2 with denormals flushed: __expf / __logf guard the denormal range with a compare and two predicated
+// multiplies each, and 1 + (a value below 2^-126) is 1 either way, so the results are the same bits
+__device__ __forceinline__ float ex2_ftz(float x) {
+  float r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+  return r;
+}
 __device__ __forceinline__ float fast_sigmoid(float x) {
   float r;
-  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + __expf(-x)));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(1.0f + ex2_ftz(x * -1.4426950408889634f)));
   return r;
 }
 __device__ __forceinline__ float fast_softplus(float x) {
-  return x > 20.0f ? x : __logf(1.0f + __expf(x));
+  float l;
+  asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l) : "f"(1.0f + ex2_ftz(x * 1.4426950408889634f)));
+  return x > 20.0f ? x : l * 0.6931471805599453f;        // a select, not a branch
 }
 
 // trunk-1 A row: [F(q) (63), 1] as 32 bf16x2 words, generated level by level with the double-angle
