@@ -205,6 +205,8 @@ def time_config(r360, config, precision, steps=5, warmup=3, pinhole=None):
            "ms_mlp": ms_mlp, "chunks": int(st.chunks)}
     if precision == "bf16":
         out["mlp_frac_of_bf16_sustained"] = st.samples_emitted * fl / (ms_mlp * 1e-3) / 1e12 / peaks["bf16_sustained"]
+        # the sustained figure is cuBLAS under its own power throttle; a kernel that holds the full clock can pass it
+        out["mlp_frac_of_bf16_burst"] = st.samples_emitted * fl / (ms_mlp * 1e-3) / 1e12 / peaks["bf16"]
     scene.close()
     del rgb, depth, flush
     torch.cuda.empty_cache()
@@ -363,6 +365,10 @@ def main():
         if precision == "bf16" and args.config == 3:
             roof["traffic"] = ncu_traffic("k_mlp_tc")
         if precision == "bf16":
+            # MEASURED_PEAKS.json's sustained figure is a power-throttled cuBLAS run (its clocks_under_load block);
+            # the fraction of the burst figure is reported beside it
+            roof["peak_burst"] = peaks["bf16"]
+            roof["frac_of_burst"] = ach / peaks["bf16"]
             roof["executed_flop_per_sample"] = executed_flop_per_sample(sc.hidden_width, sc.n_hidden)
         roof["samples_per_launch"] = int(samples)
         roof["ms_per_launch"] = ms_mlp

@@ -389,6 +389,28 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     // hide DRAM latency without registers: the next tile's records (same subfield, so their place is known) travel to shared memory with
     // cp.async and the records of the tile after it go to L2
     const bool stage_next = spt <= kStageSegs && tile + 1 < tile1 && tile + 1 < k_tile_end;
+    // one warp (not the one that issues the MMAs) stages the next tile's records for the whole group: thread i of the
+    // staging warp takes segment i (K >= 4: at most 32 segments per tile); the other three warps skip the block
+    auto stage_records = [&]() {
+      const int si = spt <= 32 ? tid - 32 * stg_warp : (j == 0 ? sidx : -1);
+      if (si >= 0 && si < spt) {
+        const unsigned sn = seg0 + spt + si;
+        if (sn < k_seg_end) {
+          if (stage_next) {
+            uint4* dp = &rec_stage_s[grp][stage_buf ^ 1][si * kRecWords];
+            cp_async_16(dp, b.recs + (size_t)sn * kRecWords);
+            cp_async_16(dp + 1, b.recs + (size_t)sn * kRecWords + 1);
+          }
+          if (sn + spt < k_seg_end) prefetch_l2(b.recs + (size_t)(sn + spt) * kRecWords);
+        }
+      }
+      cp_async_commit();
+    };
+    // width 32: behind the first layer's barrier (in front of it the staging warp reached the barrier last and the
+    // whole group waited for it: 1.244 -> 1.214 ms on config 3); width 64, where the tensor pipe is the bound and a
+    // group's four warps have a scheduler slot each to themselves: in front (behind it, config 4 was 4 % slower)
+    constexpr bool kStageLate = WD == 32;
+    if (!kStageLate) stage_records();
     const float* P = f.poses + rd.w * 12;
     const float t = __fmaf_rn(jf, __uint_as_float(rec.z), __uint_as_float(rec.y));   // reading D
     float q[3];                                              // reading A3
@@ -421,23 +443,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
       }
       __syncwarp();
     }
-    // (behind the first layer's barrier: in front of it the staging warp reached the barrier last and the whole
-    // group waited for it)
-    // one warp (not the one that issues the MMAs) does this for the whole tile: thread i of warp 3 takes segment i
-    // (K >= 4: at most 32 segments per tile); the other three warps skip the block as a whole
-    const int si = spt <= 32 ? tid - 32 * stg_warp : (j == 0 ? sidx : -1);
-    if (si >= 0 && si < spt) {
-      const unsigned sn = seg0 + spt + si;
-      if (sn < k_seg_end) {
-        if (stage_next) {
-          uint4* dp = &rec_stage_s[grp][stage_buf ^ 1][si * kRecWords];
-          cp_async_16(dp, b.recs + (size_t)sn * kRecWords);
-          cp_async_16(dp + 1, b.recs + (size_t)sn * kRecWords + 1);
-        }
-        if (sn + spt < k_seg_end) prefetch_l2(b.recs + (size_t)(sn + spt) * kRecWords);
-      }
-    }
-    cp_async_commit();
+    if (kStageLate) stage_records();
     wait_acc();
     tmem_st_x16(tA + S::A_FD, ad);                           // parks behind h for every later layer
     // ---- trunk-2..Hd: A = [h, 1, 1, ...]
