@@ -449,6 +449,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     // ---- trunk-2..Hd: A = [h, 1, 1, ...]
     // (the loop runs on the descriptor itself: its end value is already in a uniform register, a comparison with
     // net.Hd would put a parameter load between the accumulator wait and the tcgen05.ld of the next layer)
+#pragma unroll 1
     for (uint32_t dlt = dl0 + kT1; dlt != dlc; dlt += kTS) {
       d_to_a(tA + S::A_H);
       publish();
