@@ -296,7 +296,8 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   uint32_t par_d = 0, par_w = 0;
   const int K = g.K;
   const int sidx = tid / K, j = tid - sidx * K;
-  const float jf = (float)j + 0.5f;
+  float jf = (float)j + 0.5f;
+  asm volatile("" : "+f"(jf));              // kept in its register: ptxas otherwise rebuilds it from the thread index in every tile
 
   // MMAs of one operand pair: ks K steps, A from TMEM columns a_col.., B blocks of N rows at b_off
   // The group's weight buffer never moves, so a block's descriptor is the buffer's plus the block's offset in
@@ -502,7 +503,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     uint2 o2;
     o2.x = pack_f16(sigma, fast_sigmoid(__uint_as_float(craw[0]) + hb.x));
     o2.y = pack_f16(fast_sigmoid(__uint_as_float(craw[1]) + hb.y), fast_sigmoid(__uint_as_float(craw[2]) + hb.z));
-    if (active) reinterpret_cast<uint2*>(b.out)[(size_t)rec.w * K + j] = o2;
+    if (active) reinterpret_cast<uint2*>(b.out)[(size_t)rec.w * K + __float2int_rz(jf)] = o2;
   }
   fence_before_sync();
   __syncthreads();
