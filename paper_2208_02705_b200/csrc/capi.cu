@@ -196,6 +196,7 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
   }
   g.K = desc->samples_per_voxel;
   g.Kf = (float)g.K;
+  g.Kinv = (g.K > 0 && (g.K & (g.K - 1)) == 0) ? 1.0f / (float)g.K : 0.0f;
   sc->segs_per_tile = kTileRows / g.K;
   NetShape& net = sc->net;
   net.Wd = Wd; net.Hd = desc->n_hidden; net.Lp = desc->pe_pos_levels; net.Ld = desc->pe_dir_levels;

@@ -116,7 +116,7 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
       if (cnt < kHitCap) {
         // reading D: delta = (t_out - t_in) / K, one subtract, one divide
         const size_t h = (size_t)cnt * f.n_rays + r;
-        b.hit_t[h] = make_float2(t_in, __fdiv_rn(__fsub_rn(t_out, t_in), g.Kf));
+        b.hit_t[h] = make_float2(t_in, seg_delta(g, t_in, t_out));
         b.hit_lab[h] = (uint16_t)lab;
       }
       ++cnt;
@@ -350,7 +350,7 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
         --skip;
         hit = false;
       }
-      if (hit) dt = __fdiv_rn(__fsub_rn(t_out, t_in), g.Kf);    // reading D
+      if (hit) dt = seg_delta(g, t_in, t_out);    // reading D
       more = w.alive;
     }
     unsigned m = __ballot_sync(0xffffffffu, hit);
