@@ -12,6 +12,6 @@ multi-room indoor floors, camera about 1 m above the floor, n from 16 to ~4000
 tiny 32/64-wide MLPs).  Recipe: DESIGN.md "Input recipe".
 """
 from .rng import SplitMix64
-from .scenes import CONFIGS, Scene, make_scene, mlp_param_count, weight_layout
+from .scenes import CONFIGS, Scene, make_nondyadic_scene, make_scene, mlp_param_count, weight_layout
 
-__all__ = ["SplitMix64", "CONFIGS", "Scene", "make_scene", "mlp_param_count", "weight_layout"]
+__all__ = ["SplitMix64", "CONFIGS", "Scene", "make_scene", "make_nondyadic_scene", "mlp_param_count", "weight_layout"]

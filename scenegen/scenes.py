@@ -343,3 +343,58 @@ def make_scene(config: int, with_weights: bool = True) -> Scene:
                  samples_per_voxel=cfg["K"], t_threshold=1e-3, density_activation=1,
                  occ_threshold=OCC_THRESHOLD, occupancy=val, voxel_subfield=labels, weights=weights,
                  poses=poses)
+
+
+# --------------------------------------------------------------------------- parity-test scene (not a BASELINE.json config)
+
+def make_nondyadic_scene(seed: int = 100, K: int = 5, n: int = 7, occupancy_fraction: float = 0.12,
+                         W: int = 96, H: int = 48) -> Scene:
+    """Non-dyadic, anisotropic test scene: box [-1.3, 2.07] x [0.2, 3.9] x [-0.7, 1.13], grid 37 x 29 x 11
+    (voxel sizes 0.0911 / 0.1276 / 0.1664 m, none a power of two, box_min not representable in binary32), random
+    scattered occupancy (no shell: many rays leave the grid through empty space), kd-split labels, Xavier
+    weights, a camera that sits on no lattice plane with a general (not gravity-aligned) rotation, and K = 5
+    (not a power of two).  The BASELINE.json configs all have power-of-two voxel sizes and exactly
+    representable planes, which would hide a contracted or reordered plane formula in a walk; this one does not.
+    Pose 0: camera in free space; pose 1: camera inside an occupied voxel; pose 2: camera outside the box."""
+    dims = (37, 29, 11)
+    box_min, box_max = (-1.3, 0.2, -0.7), (2.07, 3.9, 1.13)
+    nx, ny, nz = dims
+    vs = (np.array(box_max) - np.array(box_min)) / np.array(dims, dtype=np.float64)
+    rng = SplitMix64(seed, _S_BOXES)
+    occ = (rng.uniform(nx * ny * nz) < occupancy_fraction).reshape(nz, ny, nx)
+    # a few solid blobs so that rays cross runs of adjacent occupied voxels as well as isolated ones
+    for _ in range(6):
+        u = rng.uniform(6)
+        e = 1 + (u[:3] * np.array([6, 5, 3])).astype(int)
+        x0, y0, z0 = (u[3:] * (np.array(dims) - e)).astype(int)
+        occ[z0:z0 + e[2], y0:y0 + e[1], x0:x0 + e[0]] = True
+    labels = _kd_split(occ, vs, n)
+    r = SplitMix64(seed, _S_OCCVAL).bits(occ.size)
+    val = np.where(occ.reshape(-1), OCC_THRESHOLD + (r % np.uint64(8)), r % np.uint64(41)).astype(np.uint8)
+    cfg = dict(width=32, n_hidden=2, sigma_bias=1.0)
+    weights = _build_weights(cfg, seed, n)
+    # general rotation from a seeded unit quaternion
+    pr = SplitMix64(seed, _S_POSE)
+    q = pr.uniform(4) * 2.0 - 1.0
+    q /= np.linalg.norm(q)
+    a, b, c, d = q
+    R = np.array([[a * a + b * b - c * c - d * d, 2 * (b * c - a * d), 2 * (b * d + a * c)],
+                  [2 * (b * c + a * d), a * a - b * b + c * c - d * d, 2 * (c * d - a * b)],
+                  [2 * (b * d - a * c), 2 * (c * d + a * b), a * a - b * b - c * c + d * d]])
+    flat = occ.reshape(-1)
+    free = np.flatnonzero(~flat)
+    full = np.flatnonzero(flat)
+
+    def centre_of(lin, frac):
+        idx = np.array([lin % nx, (lin // nx) % ny, lin // (nx * ny)], dtype=np.float64)
+        return np.array(box_min) + (idx + frac) * vs
+
+    o_free = centre_of(int(free[int(pr.uniform1() * free.size)]), np.array([0.37, 0.61, 0.43]))
+    o_occ = centre_of(int(full[int(pr.uniform1() * full.size)]), np.array([0.53, 0.29, 0.71]))
+    o_out = np.array([box_min[0] - 0.77, box_max[1] + 0.31, 0.5 * (box_min[2] + box_max[2]) + 0.113])
+    poses = np.stack([np.concatenate([R, o.reshape(3, 1)], axis=1).astype(np.float32).reshape(12)
+                      for o in (o_free, o_occ, o_out)])
+    return Scene(config=0, name="nondyadic", W=W, H=H, dims=dims, box_min=box_min, box_max=box_max, n_subfields=n,
+                 hidden_width=32, n_hidden=2, pe_pos_levels=10, pe_dir_levels=4, samples_per_voxel=K,
+                 t_threshold=1e-3, density_activation=1, occ_threshold=OCC_THRESHOLD, occupancy=val,
+                 voxel_subfield=labels, weights=weights, poses=poses)
