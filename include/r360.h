@@ -157,7 +157,17 @@ r360_status r360_set_camera(r360_scene* scene, int32_t model, double fx, double 
  * r360_stats.segments / mlp_tiles count what reached the MLP, and the per-stage times cover the first pass. */
 r360_status r360_set_wavefront(r360_scene* scene, int32_t enable);
 
-/* 0 = fp32 MLP on the FP32 ALUs (default); 1 = bf16 tensor-core MLP (tcgen05, fp32 accumulate). */
+/* Arithmetic of the tiny MLPs (steps a6-a9; Eq.1, Table 4):
+ *  0 = binary32 on the FP32 ALUs (default; within 1e-4 of the oracle);
+ *  1 = tensor cores (tcgen05), operands (weights, positional encoding, activations) rounded to bfloat16,
+ *      binary32 accumulation -- BASELINE.json's "bf16 tensor-core variant";
+ *  2 = the same kernel with binary16 operands (11 significant bits instead of 8, same speed): the mode for scenes
+ *      whose pixels are decided by one or two samples (opaque surfaces), where bfloat16's per-sample colour error
+ *      (up to 2.4e-3) is not averaged out; DESIGN.md section 6 has the per-layer error table.
+ * R360_ERR_INVALID_ARG: unknown mode; modes 1-2 for a network the tensor kernel does not cover (positional
+ * encodings other than L = 10 / 4, or weight buffers that exceed the SM's shared memory: Wd = 32 with more than 6
+ * trunk layers, Wd = 64 with more than 3); mode 2 when a weight, a bias or a product of the folded feature and
+ * colour layers exceeds binary16's range (65504). */
 r360_status r360_set_precision(r360_scene* scene, int32_t mode);
 /* CUDA stream (cudaStream_t / CUstream as void*) all work of this scene is enqueued on. */
 r360_status r360_set_stream(r360_scene* scene, void* cuda_stream);

@@ -208,7 +208,8 @@ class Scene:
         self.close()
 
     def set_precision(self, mode):
-        _check(lib().r360_set_precision(self._h, {"fp32": 0, "bf16": 1}.get(mode, mode)), "r360_set_precision")
+        """"fp32" (FP32 ALUs), "bf16" (tensor cores, bfloat16 operands) or "f16" (tensor cores, binary16 operands)."""
+        _check(lib().r360_set_precision(self._h, {"fp32": 0, "bf16": 1, "f16": 2}.get(mode, mode)), "r360_set_precision")
 
     def set_wavefront(self, enable):
         _check(lib().r360_set_wavefront(self._h, int(bool(enable))), "r360_set_wavefront")

@@ -81,7 +81,8 @@ r360_status r360_cuda_fail(cudaError_t e, const char* what) {
 namespace r360 {
 // defined in mlp_tc.cu: bf16 operand packing for the tensor-core kernel
 size_t tc_pack_stride(const NetShape& net);
-void tc_pack_subfield(const NetShape& net, const float* src_blob, void* dst);
+bool tc_pack_subfield(const NetShape& net, const float* src_blob, void* dst, int operand_f16);
+size_t tc_smem_bytes(const NetShape& net);
 }  // namespace r360
 
 // Skip distances of the empty voxels (common.cuh: grid encoding): D = min(255, chessboard distance to
@@ -152,7 +153,7 @@ int64_t r360_params_per_subfield(const r360_scene_desc* desc) {
 
 void r360_scene_destroy(r360_scene* sc) {
   if (!sc) return;
-  cudaFree(sc->d_grid); cudaFree(sc->d_frames); cudaFree(sc->d_wt); cudaFree(sc->d_wpack);
+  cudaFree(sc->d_grid); cudaFree(sc->d_frames); cudaFree(sc->d_wt); cudaFree(sc->d_wpack); cudaFree(sc->d_wpack_f16);
   cudaFree(sc->d_tables); cudaFree(sc->d_poses);
   cudaFree(sc->buf.ray_cnt); cudaFree(sc->buf.ray_off); cudaFree(sc->buf.block_sum);
   cudaFree(sc->buf.bin_cnt); cudaFree(sc->buf.bin_start); cudaFree(sc->buf.bin_cursor);
@@ -262,11 +263,21 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
   }
   // bf16 operand tiles for the tensor-core kernel
   sc->wpack_stride = tc_pack_stride(net);
-  std::vector<unsigned char> wpack;
+  // (a network whose weight buffers do not fit the kernel's shared memory is refused at
+  // r360_set_precision, not at render time)
+  sc->tc_fits = sc->wpack_stride && tc_smem_bytes(net) <= 227 * 1024;
+  if (!sc->tc_fits) sc->wpack_stride = 0;
+  std::vector<unsigned char> wpack, wpack16;
+  bool f16_ok = true;
   if (sc->wpack_stride) {
-    try { wpack.assign((size_t)n * sc->wpack_stride, 0); } catch (const std::bad_alloc&) { return R360_ERR_OOM; }
-    for (int k = 0; k < n; ++k)
-      tc_pack_subfield(net, weights + (size_t)k * src.total, wpack.data() + (size_t)k * sc->wpack_stride);
+    try {
+      wpack.assign((size_t)n * sc->wpack_stride, 0);
+      wpack16.assign((size_t)n * sc->wpack_stride, 0);
+    } catch (const std::bad_alloc&) { return R360_ERR_OOM; }
+    for (int k = 0; k < n; ++k) {
+      tc_pack_subfield(net, weights + (size_t)k * src.total, wpack.data() + (size_t)k * sc->wpack_stride, 0);
+      f16_ok = tc_pack_subfield(net, weights + (size_t)k * src.total, wpack16.data() + (size_t)k * sc->wpack_stride, 1) && f16_ok;
+    }
   }
 
   int dev = 0;
@@ -281,6 +292,10 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
   if (!wpack.empty()) {
     R360_CUDA(cudaMalloc(&sc->d_wpack, wpack.size()));
     R360_CUDA(cudaMemcpy(sc->d_wpack, wpack.data(), wpack.size(), cudaMemcpyHostToDevice));
+    if (f16_ok) {
+      R360_CUDA(cudaMalloc(&sc->d_wpack_f16, wpack16.size()));
+      R360_CUDA(cudaMemcpy(sc->d_wpack_f16, wpack16.data(), wpack16.size(), cudaMemcpyHostToDevice));
+    }
   }
   R360_CUDA(cudaMalloc(&sc->buf.bin_cnt, (size_t)n * 4));
   R360_CUDA(cudaMalloc(&sc->buf.bin_ovf, (size_t)n * 4));

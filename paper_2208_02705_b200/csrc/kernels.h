@@ -59,7 +59,8 @@ struct ChunkBuffers {
   float4* st_c;          // [n_rays] compositing state carried between passes: C_r, C_g, C_b, D
   float* st_T;           // [n_rays] transmittance carried between passes; < 0 = the ray is finished
   // tensor path only (null otherwise):
-  uint4* dirblk;         // [n_rays*4] per ray: [1, 1, F(d), 0..] as 32 bf16 (pe.cuh)
+  uint4* dirblk;         // [n_rays*4] per ray: [1, 1, F(d), 0..] as 32 values in the operand format (pe.cuh)
+  int dir_f16;           // operand format of dirblk: 0 bfloat16, 1 binary16
 };
 
 constexpr int kSamplerThreads = 256;
@@ -90,9 +91,10 @@ cudaError_t launch_mlp_fp32(const GridParams& g, const FrameParams& f, const Chu
                             const NetShape& net, const Fp32Layout& lay, const float* weights_t,
                             const SubfieldFrame* frames, int n_bins, int segs_per_tile, int n_sms,
                             cudaStream_t s);
-// bf16 tensor-core MLP (tcgen05).  wpack: per subfield packed bf16 operand tiles + fp32 biases.
+// 16-bit tensor-core MLP (tcgen05, fp32 accumulate).  wpack: per subfield packed operand tiles (bfloat16, or
+// binary16 when operand_f16) + fp32 head biases.
 cudaError_t launch_mlp_tc(const GridParams& g, const FrameParams& f, const ChunkBuffers& b,
-                          const NetShape& net, const void* wpack, size_t wpack_stride,
+                          const NetShape& net, const void* wpack, size_t wpack_stride, int operand_f16,
                           const SubfieldFrame* frames, int n_bins, int segs_per_tile, int n_sms,
                           cudaStream_t s);
 void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,

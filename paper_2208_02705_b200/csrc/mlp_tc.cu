@@ -21,6 +21,7 @@
 // One thread per group issues the tcgen05.mma's of a layer and commits them to the group's mbarrier;
 // groups synchronise with named barriers only, so the st -> mma -> ld chains of all groups overlap.
 // Heads: reading A4 (Table 4 :438-442), biases of the two head rows added in fp32.
+#include <cmath>
 #include <cstring>
 #include <type_traits>
 #include <vector>
@@ -86,22 +87,68 @@ float bf16_value(uint16_t b) {
   std::memcpy(&f, &u, 4);
   return f;
 }
+// binary16: round to nearest even, subnormals kept, magnitudes beyond the largest finite value saturate to it
+// (tc_pack_subfield reports them, and r360_set_precision then refuses the binary16 mode)
+constexpr float kF16Max = 65504.0f;
+uint16_t f16_bits(float f) {
+  uint32_t u;
+  std::memcpy(&u, &f, 4);
+  const uint16_t sign = (uint16_t)((u >> 16) & 0x8000u);
+  const float a = std::fabs(f);
+  if (!(a <= kF16Max)) return (uint16_t)(sign | 0x7BFFu);
+  if (a < 6.103515625e-05f) {              // below 2^-14: a multiple of 2^-24, rounded to nearest even
+    const float q = a * 16777216.0f;       // exact scaling
+    const float r = std::nearbyint(q);     // default rounding mode: nearest even
+    return (uint16_t)(sign | (uint16_t)r);
+  }
+  uint32_t m = u & 0x7FFFFFFFu;
+  m += 0xFFFu + ((m >> 13) & 1u);          // round the 13 dropped mantissa bits to nearest even
+  const uint32_t h = ((m >> 13) - (112u << 10));
+  return (uint16_t)(sign | (h > 0x7BFFu ? 0x7BFFu : h));
+}
+float f16_value(uint16_t h) {
+  const uint32_t sign = (uint32_t)(h & 0x8000u) << 16;
+  const uint32_t e = (h >> 10) & 31u, m = h & 0x3FFu;
+  float v;
+  if (e == 0) {
+    v = (float)m * 5.9604644775390625e-08f;   // 2^-24
+  } else {
+    const uint32_t u = ((e + 112u) << 23) | (m << 13);
+    std::memcpy(&v, &u, 4);
+  }
+  uint32_t u;
+  std::memcpy(&u, &v, 4);
+  u |= sign;
+  std::memcpy(&v, &u, 4);
+  return v;
+}
+
+// operand format of one packing run (0 = bfloat16, 1 = binary16) and whether a value left binary16's range
+struct PackFmt {
+  int f16;
+  bool overflow;
+  uint16_t bits(float v) {
+    if (!f16) return bf16_bits(v);
+    if (std::fabs(v) > kF16Max) overflow = true;
+    return f16_bits(v);
+  }
+  float value(uint16_t b) const { return f16 ? f16_value(b) : bf16_value(b); }
+};
 
 // element (n, k) of a B operand with N rows -> halfword index inside the layer's packed bytes
 inline size_t b_index(int N, int n, int k) {
   int s = k / 16, c = (k % 16) / 8, e = k % 8, g = n / 8, r = n % 8;
   return (size_t)s * N * 16 + (size_t)g * 128 + c * 64 + r * 8 + e;
 }
-inline void put(uint16_t* dst, int N, int n, int k, float v) { dst[b_index(N, n, k)] = bf16_bits(v); }
-inline void put_hi_lo(uint16_t* dst, int N, int n, int k, float v) {
-  uint16_t hi = bf16_bits(v);
-  dst[b_index(N, n, k)] = hi;
-  dst[b_index(N, n, k + 1)] = bf16_bits(v - bf16_value(hi));
-}
-
 template <int WD>
-void pack_subfield_t(const NetShape& net, const float* src, void* dstv) {
+void pack_subfield_t(const NetShape& net, const float* src, void* dstv, PackFmt& fmt) {
   using S = TcShape<WD>;
+  auto put = [&fmt](uint16_t* dst, int N, int n, int k, float v) { dst[b_index(N, n, k)] = fmt.bits(v); };
+  auto put_hi_lo = [&fmt](uint16_t* dst, int N, int n, int k, float v) {
+    const uint16_t hi = fmt.bits(v);
+    dst[b_index(N, n, k)] = hi;
+    dst[b_index(N, n, k + 1)] = fmt.bits(v - fmt.value(hi));
+  };
   TcLayout L = make_tc_layout<WD>(net.Hd);
   std::memset(dstv, 0, (size_t)L.total);
   unsigned char* dst = (unsigned char*)dstv;
@@ -170,9 +217,12 @@ size_t tc_pack_stride(const NetShape& net) {
   return 0;
 }
 
-void tc_pack_subfield(const NetShape& net, const float* src_blob, void* dst) {
-  if (net.Wd == 32) pack_subfield_t<32>(net, src_blob, dst);
-  else if (net.Wd == 64) pack_subfield_t<64>(net, src_blob, dst);
+// operand_f16: 0 = bfloat16 operands, 1 = binary16 operands.  Returns false if a value does not fit binary16.
+bool tc_pack_subfield(const NetShape& net, const float* src_blob, void* dst, int operand_f16) {
+  PackFmt fmt{operand_f16, false};
+  if (net.Wd == 32) pack_subfield_t<32>(net, src_blob, dst, fmt);
+  else if (net.Wd == 64) pack_subfield_t<64>(net, src_blob, dst, fmt);
+  return !fmt.overflow;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -199,6 +249,7 @@ __device__ __forceinline__ float fast_softplus(float x) {
 
 // trunk-1 A row: [F(q) (63), 1] as 32 bf16x2 words, generated level by level with the double-angle
 // recurrence and stored K step by K step (16 values = 8 TMEM columns), so that few values are live.
+template <bool F16>
 __device__ __forceinline__ void store_pe_row(uint32_t tA, const float q[3]) {
   // The row holds sin and TWICE the cosine of every level (the host halves the matching weight columns, which is
   // exact in bf16), because the double-angle step on (s, g = 2c) is s' = g s, g' = g g - 2: two operations per
@@ -235,13 +286,13 @@ __device__ __forceinline__ void store_pe_row(uint32_t tA, const float q[3]) {
     if ((idx & 15) == 15) {
       uint32_t a8[8];
 #pragma unroll
-      for (int p = 0; p < 8; ++p) a8[p] = pack_bf16(buf[2 * p], buf[2 * p + 1]);
+      for (int p = 0; p < 8; ++p) a8[p] = pack16<F16>(buf[2 * p], buf[2 * p + 1]);
       tmem_st_x8(tA + 8 * (idx >> 4), a8);
     }
   }
 }
 
-template <int WD>
+template <int WD, bool F16>
 __global__ void __launch_bounds__(TcShape<WD>::kGroups * kTileRows, 1)
 k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay,
          const unsigned char* __restrict__ wpack, const SubfieldFrame* __restrict__ frames, int n_bins,
@@ -287,7 +338,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   const uint32_t mA = tbase + colG, mD = mA + S::D0;           // MMA operand addresses (lane 0)
 
   const uint32_t sw_addr = smem_u32(sw);
-  const uint32_t idesc_w = instr_desc_bf16(128, WD), idesc_h = instr_desc_bf16(128, S::NHEAD);
+  const uint32_t idesc_w = instr_desc_16(128, WD, F16), idesc_h = instr_desc_16(128, S::NHEAD, F16);
   const uint32_t bar_id = (uint32_t)grp + 1;
   // warp w of every group runs on scheduler w.  The warp that issues the MMAs and the one that stages the next
   // tile's records carry extra instructions, so both roles rotate with the group: each scheduler then hosts the
@@ -336,7 +387,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
       wait_ld();
       uint32_t a[16];
 #pragma unroll
-      for (int c = 0; c < 16; ++c) a[c] = pack_bf16_relu(__uint_as_float(d[2 * c]), __uint_as_float(d[2 * c + 1]));
+      for (int c = 0; c < 16; ++c) a[c] = pack16_relu<F16>(__uint_as_float(d[2 * c]), __uint_as_float(d[2 * c + 1]));
       tmem_st_x16(dst + h / 2, a);
     }
   };
@@ -421,7 +472,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
     if (!active) q[0] = q[1] = q[2] = 0.0f;                  // idle rows stay finite
 
     // ---- trunk-1: A = [F(q), 1]
-    store_pe_row(tA, q);
+    store_pe_row<F16>(tA, q);
     // the ray's direction block [1, 1, F(d), 0 0 0]: requested before the group barrier so that the load runs
     // behind the barrier, the MMA issue and the MMA itself (asked for after the issue it arrived later than the
     // accumulators: 4 % of the kernel's stall samples sat on the tcgen05.st below)
@@ -510,7 +561,7 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   if (threadIdx.x < 32) tmem_dealloc<512>(tbase);
 }
 
-template <int WD>
+template <int WD, bool F16>
 static cudaError_t launch_tc_t(const GridParams& g, const FrameParams& f, const ChunkBuffers& b,
                                const NetShape& net, const void* wpack, const SubfieldFrame* frames, int n_bins,
                                int spt, int n_sms, cudaStream_t s) {
@@ -522,20 +573,30 @@ static cudaError_t launch_tc_t(const GridParams& g, const FrameParams& f, const 
   size_t smem = (size_t)S::kGroups * lay.total;
   if (smem < 120 * 1024) smem = 120 * 1024;
   if (smem > 227 * 1024) return cudaErrorInvalidValue;
-  cudaError_t e = cudaFuncSetAttribute(k_mlp_tc<WD>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaError_t e = cudaFuncSetAttribute(k_mlp_tc<WD, F16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   if (e != cudaSuccess) return e;
-  k_mlp_tc<WD><<<n_sms, S::kGroups * kTileRows, smem, s>>>(g, f, b, net, lay, (const unsigned char*)wpack, frames,
-                                                          n_bins, spt);
+  k_mlp_tc<WD, F16><<<n_sms, S::kGroups * kTileRows, smem, s>>>(g, f, b, net, lay, (const unsigned char*)wpack, frames,
+                                                               n_bins, spt);
   return cudaGetLastError();
 }
 
 cudaError_t launch_mlp_tc(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, const NetShape& net,
-                          const void* wpack, size_t wpack_stride, const SubfieldFrame* frames, int n_bins,
-                          int segs_per_tile, int n_sms, cudaStream_t s) {
+                          const void* wpack, size_t wpack_stride, int operand_f16, const SubfieldFrame* frames,
+                          int n_bins, int segs_per_tile, int n_sms, cudaStream_t s) {
   if (!wpack || wpack_stride == 0) return cudaErrorNotSupported;
-  if (net.Wd == 32) return launch_tc_t<32>(g, f, b, net, wpack, frames, n_bins, segs_per_tile, n_sms, s);
-  if (net.Wd == 64) return launch_tc_t<64>(g, f, b, net, wpack, frames, n_bins, segs_per_tile, n_sms, s);
+  if (net.Wd == 32 && !operand_f16) return launch_tc_t<32, false>(g, f, b, net, wpack, frames, n_bins, segs_per_tile, n_sms, s);
+  if (net.Wd == 32) return launch_tc_t<32, true>(g, f, b, net, wpack, frames, n_bins, segs_per_tile, n_sms, s);
+  if (net.Wd == 64 && !operand_f16) return launch_tc_t<64, false>(g, f, b, net, wpack, frames, n_bins, segs_per_tile, n_sms, s);
+  if (net.Wd == 64) return launch_tc_t<64, true>(g, f, b, net, wpack, frames, n_bins, segs_per_tile, n_sms, s);
   return cudaErrorInvalidValue;
+}
+
+// dynamic + static shared memory the tensor kernel needs for this network; 0 if the tensor path does not apply
+size_t tc_smem_bytes(const NetShape& net) {
+  if (net.Lp != kLp || net.Ld != kLd) return 0;
+  if (net.Wd == 32) return (size_t)TcShape<32>::kGroups * make_tc_layout<32>(net.Hd).total + 20 * 1024;
+  if (net.Wd == 64) return (size_t)TcShape<64>::kGroups * make_tc_layout<64>(net.Hd).total + 12 * 1024;
+  return 0;
 }
 
 }  // namespace r360

@@ -29,6 +29,24 @@ __device__ __forceinline__ uint32_t pack_f16(float lo, float hi) {
   return r;
 }
 
+// same with ReLU fused into the conversion; out-of-range magnitudes saturate to the largest finite binary16 value
+__device__ __forceinline__ uint32_t pack_f16_relu(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.relu.satfinite.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+// operand format of the tensor path: F16 = false bfloat16, true binary16
+template <bool F16>
+__device__ __forceinline__ uint32_t pack16(float lo, float hi) {
+  if constexpr (F16) return pack_f16(lo, hi);
+  else return pack_bf16(lo, hi);
+}
+template <bool F16>
+__device__ __forceinline__ uint32_t pack16_relu(float lo, float hi) {
+  if constexpr (F16) return pack_f16_relu(lo, hi);
+  else return pack_bf16_relu(lo, hi);
+}
+
 // packed binary32 pairs (sm_100: add / mul / fma .f32x2 on a 64-bit register pair)
 __device__ __forceinline__ uint64_t pack_f32x2(float lo, float hi) {
   uint64_t r;
@@ -146,22 +164,29 @@ __device__ __forceinline__ void pe_recurrence(const float x[3], float* out) {
   }
 }
 
-// Per-ray direction block of the tensor path (64 bytes = 32 bf16): [1, 1, F(d) (27), 0, 0, 0].
+// Per-ray direction block of the tensor path (64 bytes = 32 values in the operand format): [1, 1, F(d) (27), 0, 0, 0].
 // It is the tail of the A operand of every layer after the first: the two ones feed the bias hi/lo
 // rows of the hidden layers (first 16 entries = one K step), the whole block feeds the colour layer.
 constexpr int kDirBlockWords = 16;
 
-__device__ __forceinline__ void store_dir_block(uint4* dst, const float d[3]) {
+__device__ __forceinline__ void store_dir_block(uint4* dst, const float d[3], bool f16) {
   float pd[32];
   pd[0] = 1.0f;
   pd[1] = 1.0f;
   pe_recurrence<kTcLd>(d, pd + 2);
 #pragma unroll
   for (int c = 2 + kTcPeD; c < 32; ++c) pd[c] = 0.0f;
+  if (f16) {
 #pragma unroll
-  for (int c = 0; c < 4; ++c)
-    dst[c] = make_uint4(pack_bf16(pd[8 * c], pd[8 * c + 1]), pack_bf16(pd[8 * c + 2], pd[8 * c + 3]),
-                        pack_bf16(pd[8 * c + 4], pd[8 * c + 5]), pack_bf16(pd[8 * c + 6], pd[8 * c + 7]));
+    for (int c = 0; c < 4; ++c)
+      dst[c] = make_uint4(pack_f16(pd[8 * c], pd[8 * c + 1]), pack_f16(pd[8 * c + 2], pd[8 * c + 3]),
+                          pack_f16(pd[8 * c + 4], pd[8 * c + 5]), pack_f16(pd[8 * c + 6], pd[8 * c + 7]));
+  } else {
+#pragma unroll
+    for (int c = 0; c < 4; ++c)
+      dst[c] = make_uint4(pack_bf16(pd[8 * c], pd[8 * c + 1]), pack_bf16(pd[8 * c + 2], pd[8 * c + 3]),
+                          pack_bf16(pd[8 * c + 4], pd[8 * c + 5]), pack_bf16(pd[8 * c + 6], pd[8 * c + 7]));
+  }
 }
 
 }  // namespace r360

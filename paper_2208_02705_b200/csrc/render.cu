@@ -104,9 +104,10 @@ r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::Chunk
   if ((st = grow(sc->buf.block_sum, sc->blocks_cap, n_blocks, 1, 1)) != R360_OK) return st;
   if ((st = grow(sc->buf.hit_t, sc->hit_t_cap, (size_t)f.n_rays * kHitCap, 1, 1)) != R360_OK) return st;
   if ((st = grow(sc->buf.hit_lab, sc->hit_lab_cap, (size_t)f.n_rays * kHitCap, 1, 1)) != R360_OK) return st;
-  if (sc->precision == 1) {            // tensor path: per-ray records (direction + packed F(d))
+  if (sc->precision >= 1) {            // tensor path: per-ray records (direction + packed F(d))
     if ((st = grow(sc->d_dirblk, sc->dirblk_cap, (size_t)f.n_rays * 4, 1, 1)) != R360_OK) return st;
     sc->buf.dirblk = sc->d_dirblk;
+    sc->buf.dir_f16 = sc->precision == 2;
   } else {
     sc->buf.dirblk = nullptr;
   }
@@ -198,9 +199,10 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
         // per-sample MLP outputs: K * segments float4, ray-major
         if ((st = grow(sc->buf.out, sc->out_cap, (size_t)n_segs * sc->grid_p.K)) != R360_OK) return st;
         cudaError_t e;
-        if (sc->precision == 1)
-          e = launch_mlp_tc(sc->grid_p, f, sc->buf, sc->net, sc->d_wpack, sc->wpack_stride, sc->d_frames,
-                            sc->desc.n_subfields, sc->segs_per_tile, sc->n_sms, s);
+        if (sc->precision >= 1)
+          e = launch_mlp_tc(sc->grid_p, f, sc->buf, sc->net, sc->precision == 2 ? sc->d_wpack_f16 : sc->d_wpack,
+                            sc->wpack_stride, sc->precision == 2, sc->d_frames, sc->desc.n_subfields,
+                            sc->segs_per_tile, sc->n_sms, s);
         else
           e = launch_mlp_fp32(sc->grid_p, f, sc->buf, sc->net, sc->lay, sc->d_wt, sc->d_frames,
                               sc->desc.n_subfields, sc->segs_per_tile, sc->n_sms, s);
@@ -208,7 +210,7 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
         launches += 1;
       }
       if (pev) cudaEventRecord(pev->e[4], s);
-      launch_composite(sc->grid_p, f, sc->buf, sc->desc.t_threshold, out_rgb, out_depth, pp, sc->precision == 1, s);
+      launch_composite(sc->grid_p, f, sc->buf, sc->desc.t_threshold, out_rgb, out_depth, pp, sc->precision >= 1, s);
       launches += 1;
       R360_CUDA(cudaGetLastError());
       if (pev) cudaEventRecord(pev->e[5], s);
@@ -270,8 +272,9 @@ r360_status r360_render_batch_host(r360_scene* sc, const float* poses, int32_t B
 }
 
 r360_status r360_set_precision(r360_scene* sc, int32_t mode) {
-  if (!sc || (mode != 0 && mode != 1)) return R360_ERR_INVALID_ARG;
+  if (!sc || mode < 0 || mode > 2) return R360_ERR_INVALID_ARG;
   if (mode == 1 && !sc->d_wpack) return R360_ERR_INVALID_ARG;
+  if (mode == 2 && !sc->d_wpack_f16) return R360_ERR_INVALID_ARG;
   sc->precision = mode;
   return R360_OK;
 }

@@ -100,7 +100,7 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
   if (valid) {
     const Ray ray = make_ray(f, r);
     w.init(g, ray);
-    if (b.dirblk) store_dir_block(b.dirblk + (size_t)r * 4, ray.d);   // tensor path: F(d) once per ray
+    if (b.dirblk) store_dir_block(b.dirblk + (size_t)r * 4, ray.d, b.dir_f16 != 0);   // tensor path: F(d) once per ray
   }
   uint32_t cnt = 0;
   // lock-step over "next occupied voxel" so the histogram update can be warp-aggregated

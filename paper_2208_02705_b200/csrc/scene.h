@@ -16,8 +16,10 @@ struct r360_scene {
   uint16_t* d_grid = nullptr;               // fused occupancy + label + skip distance (common.cuh)
   r360::SubfieldFrame* d_frames = nullptr;  // [n]
   float* d_wt = nullptr;                    // [n * lay.total] fp32, transposed + padded
-  void* d_wpack = nullptr;                  // [n * wpack_stride] bf16 operand tiles + fp32 biases
+  void* d_wpack = nullptr;                  // [n * wpack_stride] bfloat16 operand tiles + fp32 head biases
+  void* d_wpack_f16 = nullptr;              // the same in binary16; null if a weight does not fit binary16
   size_t wpack_stride = 0;
+  bool tc_fits = false;                     // the tensor kernel's shared memory fits this network
   // per (W,H): trig tables; per call: poses
   float* d_tables = nullptr;
   int tab_W = 0, tab_H = 0;
@@ -42,7 +44,7 @@ struct r360_scene {
   cudaEvent_t ev_chunk_done = nullptr;
   // configuration
   cudaStream_t stream = nullptr;
-  int precision = 0;
+  int precision = 0;                        // 0 fp32 ALUs, 1 tensor cores bfloat16, 2 tensor cores binary16
   int wavefront = 0;                        // r360_set_wavefront: feed the MLP in passes, retire finished rays between them
   uint32_t* d_pass_cnt = nullptr;           // owned; buf.pass_cnt points here only during wavefront passes
   size_t pass_cnt_cap = 0, pass_off_cap = 0, st_c_cap = 0, st_T_cap = 0;

@@ -122,13 +122,13 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes
   d |= (uint64_t)1 << 46;   // descriptor version 1 (sm_100)
   return d;                 // base_offset 0, lbo_mode 0, layout_type 0 = SWIZZLE_NONE
 }
-// Instruction descriptor, kind::f16: D fp32, A/B bf16, both K-major, dense.
-__host__ __device__ constexpr uint32_t instr_desc_bf16(int M, int N) {
-  return (1u << 4)                     // c_format  = F32
-         | (1u << 7)                   // a_format  = BF16
-         | (1u << 10)                  // b_format  = BF16
-         | ((uint32_t)(N >> 3) << 17)  // n_dim
-         | ((uint32_t)(M >> 4) << 24); // m_dim
+// Instruction descriptor, kind::f16: D fp32, A/B bfloat16 (format 1) or binary16 (format 0), both K-major, dense.
+__host__ __device__ constexpr uint32_t instr_desc_16(int M, int N, bool f16) {
+  return (1u << 4)                           // c_format  = F32
+         | ((f16 ? 0u : 1u) << 7)            // a_format
+         | ((f16 ? 0u : 1u) << 10)           // b_format
+         | ((uint32_t)(N >> 3) << 17)        // n_dim
+         | ((uint32_t)(M >> 4) << 24);       // m_dim
 }
 
 // ---- MMA: D[tmem] (+)= A[tmem] * B[smem]^T   (one thread issues for the CTA) -----------------

@@ -1,6 +1,7 @@
-"""-m gpu: the bf16 tensor-core MLP path (tcgen05) against the oracle: RGB within 2e-3 absolute,
-max over pixels (BASELINE.json north_star).  Depth is a sum of w_i * t_i with t up to the scene
-diagonal, so its bound scales with the ray length: 2e-3 * t_max."""
+"""-m gpu: the tensor-core MLP path (tcgen05; bfloat16 operands = BASELINE.json's "bf16 tensor-core variant", and
+the same kernel with binary16 operands) against the oracle: RGB within 2e-3 absolute, max over pixels
+(BASELINE.json north_star).  Depth is a sum of w_i * t_i with t up to the scene diagonal, so its bound scales
+with the ray length: 2e-3 * t_max."""
 import numpy as np
 import pytest
 
@@ -51,7 +52,7 @@ def _cmp(r360, oracle, sc, weights=None, amb_band=0.2, px=None, py=None, tol=TOL
     else:
         ref = ora.render_pixels(pose, sc.W, sc.H, px, py)
         rgb, depth = rgb[py, px], depth[py, px]
-    depth_tol = tol * _t_max(sc) if precision == "bf16" else tol
+    depth_tol = tol * _t_max(sc) if precision != "fp32" else tol
     res = check_image(rgb, depth, ref, tol, amb_band=amb_band, depth_tol=depth_tol)
     gpu.close()
     return res
@@ -64,25 +65,32 @@ def test_sass_has_tcgen05_and_tma():
     assert "UTCHMMA" in sass and "LDTM" in sass and "STTM" in sass and "UBLKCP" in sass
 
 
-def test_render_bf16_config1(r360, oracle, scene1):
-    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1)
-    print("config1 bf16 max rgb err", e_rgb, "depth", e_d)
+TC = pytest.mark.parametrize("prec", ["bf16", "f16"])
 
 
-def test_render_bf16_config2(r360, oracle, scene2):
-    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene2)
-    print("config2 bf16 max rgb err", e_rgb, "depth", e_d)
+@TC
+def test_render_tc_config1(r360, oracle, scene1, prec):
+    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, precision=prec)
+    print("config1", prec, "max rgb err", e_rgb, "depth", e_d)
 
 
+@TC
+def test_render_tc_config2(r360, oracle, scene2, prec):
+    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene2, precision=prec)
+    print("config2", prec, "max rgb err", e_rgb, "depth", e_d)
+
+
+@TC
 @pytest.mark.parametrize("over", [dict(samples_per_voxel=12), dict(samples_per_voxel=5),
                                   dict(samples_per_voxel=1), dict(samples_per_voxel=16),
                                   dict(samples_per_voxel=128),
                                   dict(density_activation=0), dict(t_threshold=0.0)])
-def test_render_bf16_variants(r360, oracle, scene1, over):
-    _cmp(r360, oracle, scene1, **over)
+def test_render_tc_variants(r360, oracle, scene1, over, prec):
+    _cmp(r360, oracle, scene1, precision=prec, **over)
 
 
-def test_render_bf16_width64(r360, oracle):
+@TC
+def test_render_tc_width64(r360, oracle, prec):
     from scenegen import mlp_param_count, weight_layout
     sc = get_scene(1)
     rng = np.random.default_rng(11)
@@ -96,7 +104,7 @@ def test_render_bf16_width64(r360, oracle):
         parts.append(b)
     w = np.concatenate(parts, 1).astype(F).reshape(-1)
     assert w.size == sc.n_subfields * mlp_param_count(64, 3)
-    _cmp(r360, oracle, sc, weights=w, hidden_width=64, n_hidden=3)
+    _cmp(r360, oracle, sc, weights=w, hidden_width=64, n_hidden=3, precision=prec)
 
 
 def test_render_bf16_early_out(r360, oracle, scene1):
@@ -120,6 +128,47 @@ def test_render_bf16_saturating_density(r360, oracle, scene1, act):
     print("saturating density bf16 max rgb err", e_rgb)
 
 
+def test_render_f16_opaque_scenes(r360, oracle, scene1):
+    """The scene class the method is for (trained scenes: opaque surfaces end rays early) at
+    north_star's bar, 2e-3, on the binary16-operand tensor path: density bias 40 (every pixel is the colour of its
+    first one or two samples) and density far beyond binary16's range (sigma stored clamped to 65504, alpha = 1).
+    Ambiguity band 0.02: |dT/T| <= ln(1/tau) * max relative error of sigma = 6.9 * 2e-3."""
+    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 40.0), amb_band=0.02,
+                             tol=TOL, precision="f16")
+    print("dense stress f16 max rgb err", e_rgb, "ambiguous", n_amb)
+    for act in (0, 1):
+        e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 1.0e6), amb_band=0.02,
+                                 tol=TOL, density_activation=act, precision="f16")
+        print("saturating density f16 act", act, "max rgb err", e_rgb)
+
+
+def test_f16_refused_when_a_weight_exceeds_binary16(r360, scene1):
+    sc = scene1
+    w = sc.weights.copy()
+    w[5] = 7.0e4                      # a first-layer weight beyond 65504
+    gpu = r360.scene_from(sc, weights=w)
+    gpu.set_precision("bf16")         # bfloat16 has binary32's range
+    with pytest.raises(r360.R360Error):
+        gpu.set_precision("f16")
+    gpu.close()
+
+
+def test_tensor_path_refused_when_the_weights_exceed_shared_memory(r360, scene1):
+    # ADVICE round 1: refused at r360_set_precision, not by a failing launch at render time
+    from scenegen import mlp_param_count
+    sc = scene1
+    for width, n_hidden, ok in ((32, 6, True), (32, 7, False), (64, 3, True), (64, 4, False)):
+        P = mlp_param_count(width, n_hidden)
+        gpu = r360.scene_from(sc, weights=np.zeros(sc.n_subfields * P, F), hidden_width=width, n_hidden=n_hidden)
+        if ok:
+            gpu.set_precision("bf16")
+            gpu.render(sc.poses[0], 16, 8)
+        else:
+            with pytest.raises(r360.R360Error):
+                gpu.set_precision("bf16")
+        gpu.close()
+
+
 def test_bf16_refused_for_other_pe_sizes(r360, scene1):
     from scenegen import mlp_param_count
     sc = scene1
@@ -129,17 +178,19 @@ def test_bf16_refused_for_other_pe_sizes(r360, scene1):
         gpu.set_precision("bf16")
 
 
-def test_full_size_config3_bf16_sampled(r360, oracle):
+@TC
+def test_full_size_config3_tc_sampled(r360, oracle, prec):
     sc = get_scene(3)
     rng = np.random.default_rng(5)
     px = rng.integers(0, sc.W, 3000).astype(np.int32)
     py = rng.integers(0, sc.H, 3000).astype(np.int32)
-    e_rgb, e_d, n_amb = _cmp(r360, oracle, sc, px=px, py=py)
-    print("config3 bf16 sampled max rgb err", e_rgb, "depth", e_d)
+    e_rgb, e_d, n_amb = _cmp(r360, oracle, sc, px=px, py=py, precision=prec)
+    print("config3", prec, "sampled max rgb err", e_rgb, "depth", e_d)
 
 
+@TC
 @pytest.mark.parametrize("n_hidden", [2, 3])
-def test_render_bf16_random_biases(r360, oracle, n_hidden):
+def test_render_tc_random_biases(r360, oracle, n_hidden, prec):
     # every bias path of the tensor kernel: the single bf16 bias row of the first layer, the hi/lo rows of
     # the hidden layers, the bias of the folded feature+colour layer, the fp32 biases of the two heads
     from scenegen import mlp_param_count, weight_layout
@@ -155,9 +206,10 @@ def test_render_bf16_random_biases(r360, oracle, n_hidden):
         parts.append(b)
     w = np.concatenate(parts, 1).astype(F).reshape(-1)
     assert w.size == sc.n_subfields * mlp_param_count(32, n_hidden)
-    e_rgb, e_d, _ = _cmp(r360, oracle, sc, weights=w, n_hidden=n_hidden)
-    print("random biases, n_hidden", n_hidden, "bf16 max rgb err", e_rgb)
-    _cmp(r360, oracle, sc, weights=w, n_hidden=n_hidden, precision="fp32", tol=1e-4, amb_band=1e-3)
+    e_rgb, e_d, _ = _cmp(r360, oracle, sc, weights=w, n_hidden=n_hidden, precision=prec)
+    print("random biases, n_hidden", n_hidden, prec, "max rgb err", e_rgb)
+    if prec == "bf16":
+        _cmp(r360, oracle, sc, weights=w, n_hidden=n_hidden, precision="fp32", tol=1e-4, amb_band=1e-3)
 
 
 def _sampled(sc, n, seed):
@@ -172,6 +224,8 @@ def test_full_size_config5_sampled(r360, oracle):
     px, py = _sampled(sc, 1200, 7)
     e_rgb, e_d, _ = _cmp(r360, oracle, sc, px=px, py=py)
     print("config5 bf16 sampled max rgb err", e_rgb, "depth", e_d)
+    e_rgb, e_d, _ = _cmp(r360, oracle, sc, px=px, py=py, precision="f16")
+    print("config5 f16 sampled max rgb err", e_rgb, "depth", e_d)
     e_rgb, e_d, _ = _cmp(r360, oracle, sc, px=px, py=py, precision="fp32", tol=1e-4, amb_band=1e-3)
     print("config5 fp32 sampled max rgb err", e_rgb, "depth", e_d)
 
@@ -183,5 +237,7 @@ def test_full_size_config4_one_pose_sampled(r360, oracle):
     px, py = _sampled(sc, 1200, 9)
     e_rgb, e_d, _ = _cmp(r360, oracle, sc, px=px, py=py, pose=sc.poses[3])
     print("config4 bf16 sampled max rgb err", e_rgb, "depth", e_d)
+    e_rgb, e_d, _ = _cmp(r360, oracle, sc, px=px, py=py, pose=sc.poses[3], precision="f16")
+    print("config4 f16 sampled max rgb err", e_rgb, "depth", e_d)
     e_rgb, e_d, _ = _cmp(r360, oracle, sc, px=px, py=py, pose=sc.poses[3], precision="fp32", tol=1e-4, amb_band=1e-3)
     print("config4 fp32 sampled max rgb err", e_rgb, "depth", e_d)
