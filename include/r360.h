@@ -18,9 +18,17 @@
  *  - Every entry point returns a status; no exception or abort crosses the ABI.
  *    On failure outputs are unspecified and *out handles are NULL.
  *  - A handle may be used from one host thread at a time.
- *  - r360_render* synchronises the stream once per ray chunk internally (to size
- *    the sample buffers from the exact segment count); outputs are complete in
- *    stream order when it returns, the host need not synchronise to enqueue more.
+ *  - r360_render, r360_render_batch and r360_render_rows are ASYNCHRONOUS: they enqueue the frame on the
+ *    scene's stream and return.  The buffers that hold a frame's samples are sized from the largest
+ *    samples-per-ray ratio of earlier frames plus a quarter.  If a frame turns out to need more (a view with
+ *    over 25 % more samples per ray than any before), the kernels of the affected ray chunk do nothing and the
+ *    next call on the scene (r360_wait, r360_get_stats, any render or set call) renders that chunk again with
+ *    larger buffers, in stream order: nothing is ever truncated.  So:
+ *      - a caller that consumes the outputs through further r360 calls or after r360_get_stats needs nothing;
+ *      - a caller that consumes them in its own stream work calls r360_wait(scene) first.  It waits until the
+ *        frame's samples have been COUNTED (the first ~15 % of a frame), not for the frame, and returns
+ *        immediately in the common case;
+ *    The first frame a scene renders is sized from its exact count and waits for the GPU once per ray chunk.
  */
 #ifndef R360_H
 #define R360_H
@@ -46,6 +54,13 @@ typedef enum {
 /* Scene description.  Geometry: DESIGN.md readings C (grid planes
  * P_a(k) = box_min_a + k * (box_max_a - box_min_a)/dims_a, binary32).
  * Network: readings A1-A4 ("6212 parameters"; Table 4 :434-444). */
+/* Layout of the image outputs of the render calls (r360_set_output_format). */
+typedef enum {
+  R360_OUT_F32 = 0,      /* out_rgb float[.][3], out_depth float[.]  (default)                              */
+  R360_OUT_RGB8_D16 = 1  /* out_rgb uint8[.][3] = round(255 * clamp(C, 0, 1)), out_depth IEEE binary16[.]:   */
+                         /* 5 bytes per pixel instead of 16 for images that leave the GPU                   */
+} r360_output_format;
+
 typedef struct {
   int32_t dims[3];            /* Nx,Ny,Nz >= 1; linear voxel index = (iz*Ny+iy)*Nx+ix             */
   float box_min[3];           /* metres; box_max > box_min per axis (voxels may be anisotropic)    */
@@ -82,22 +97,57 @@ void r360_scene_destroy(r360_scene* scene);
  * Eq. 2-3) -- Eq. 2-5; steps a1-a10 of DESIGN.md.
  *  pose       HOST float[12]: row-major 3x4 [R|o], camera (x right, y down, z forward,
  *             PAPER.md:84) -> world; o = camera centre.  Must be finite.
- *  out_rgb    DEVICE float[H*W*3], row-major, black background
+ *  out_rgb    DEVICE float[H*W*3], row-major, black background   (R360_OUT_RGB8_D16: uint8[H*W*3])
  *  out_depth  DEVICE float[H*W], Eq. 4's sum w_i t_i (radial distance; not opacity-normalised)
- * Errors: INVALID_ARG (NULL, W < 1, H < 1, non-finite pose), OOM, CUDA. */
+ *             (R360_OUT_RGB8_D16: binary16[H*W])
+ * Asynchronous (see "Conventions").  Errors: INVALID_ARG (NULL, W < 1, H < 1, non-finite pose), OOM, CUDA;
+ * CAPACITY inside a CUDA stream capture when a buffer would have to be allocated (see r360_graph_status). */
 r360_status r360_render(r360_scene* scene, const float pose[12], int32_t W, int32_t H,
-                        float* out_rgb, float* out_depth);
+                        void* out_rgb, void* out_depth);
 
-/* Same for B poses (HOST float[B*12]); outputs DEVICE float[B*H*W*3], float[B*H*W]. */
+/* Same for B poses (HOST float[B*12]); outputs DEVICE [B*H*W*3], [B*H*W].  The poses of a batch are binned
+ * together, so a subfield's weights are staged once for all of them: a stereoscopic pair (PAPER.md:172-174,
+ * Fig. 5: "monoscopic ... and stereoscopic modes") is a batch of two poses one eye distance apart. */
 r360_status r360_render_batch(r360_scene* scene, const float* poses, int32_t B, int32_t W, int32_t H,
-                              float* out_rgb, float* out_depth);
+                              void* out_rgb, void* out_depth);
 
-/* End-to-end convenience: like r360_render_batch but the outputs are HOST buffers
- * (float[B*H*W*3], float[B*H*W]; pinned memory for full PCIe speed); every chunk of rays
- * (r360_set_chunk_rays) is copied device -> host on a second stream while the next chunk is
- * rendered; the call returns when all copies are done, also after an error. */
+/* A band of image rows [row0, row1) of one view: rays are independent ("each ray can be concurrently processed",
+ * PAPER.md:174), so a frame splits across GPUs by rows with no exchange but the gather of the bands (SURVEY.md
+ * 8(e)).  out_rgb / out_depth point at the BAND: DEVICE [(row1-row0)*W*3], [(row1-row0)*W]; pass
+ * frame + row0*W*3 (and frame_depth + row0*W) to render into a full-size frame in place.  The pixels are
+ * bit-identical to the same rows of r360_render.  INVALID_ARG unless 0 <= row0 < row1 <= H. */
+r360_status r360_render_rows(r360_scene* scene, const float pose[12], int32_t W, int32_t H, int32_t row0,
+                             int32_t row1, void* out_rgb, void* out_depth);
+
+/* End-to-end call: like r360_render_batch but the outputs are HOST buffers ([B*H*W*3], [B*H*W] in the
+ * scene's output format; pinned memory for full PCIe speed).  Every chunk of rays (r360_set_chunk_rays; a call
+ * that fits one chunk is cut into r360_set_host_bands bands, default 4) is copied device -> host on a second
+ * stream while the next chunk is rendered; the call returns when all copies are done, also after an error. */
 r360_status r360_render_batch_host(r360_scene* scene, const float* poses, int32_t B, int32_t W, int32_t H,
-                                   float* out_rgb_host, float* out_depth_host);
+                                   void* out_rgb_host, void* out_depth_host);
+r360_status r360_set_host_bands(r360_scene* scene, int32_t bands /* 1..64 */);
+
+/* Returns once the outputs of the last render call are guaranteed complete IN STREAM ORDER (see "Conventions"):
+ * waits for the frame's sample count, re-renders a chunk whose samples exceeded the buffers.  Does not wait for
+ * the frame itself.  Also returns the status of such a re-render (OOM, CUDA). */
+r360_status r360_wait(r360_scene* scene);
+
+/* Image output layout of the following render calls (r360_output_format).  INVALID_ARG for another value. */
+r360_status r360_set_output_format(r360_scene* scene, int32_t format);
+
+/* Pre-size the sample buffers for chunks of up to max_rays_per_chunk rays with segments_per_ray occupied voxels
+ * crossed per ray on average (x 1.25), so that no later frame has to grow them. */
+r360_status r360_reserve(r360_scene* scene, uint64_t max_rays_per_chunk, double segments_per_ray);
+
+/* CUDA graphs.  The render calls may be captured (cudaStreamBeginCapture on the scene's stream) once the scene
+ * has rendered a frame of the same size outside a capture (which builds the pixel tables and sizes the buffers;
+ * a capture that would have to allocate returns R360_ERR_CAPACITY).  The captured frame reads its poses from a
+ * pinned buffer of the scene at every replay: r360_set_graph_poses replaces them between replays (host memcpy,
+ * no CUDA call).  A replay cannot re-render a chunk that outgrew the buffers: r360_graph_status synchronises the
+ * stream and returns R360_ERR_CAPACITY if the last replay hit that case (its outputs are then incomplete; call
+ * r360_reserve with a larger ratio and capture again), R360_OK otherwise. */
+r360_status r360_set_graph_poses(r360_scene* scene, const float* poses, int32_t B);
+r360_status r360_graph_status(r360_scene* scene);
 
 /* Algorithm 1, stage II (text :157): geometry-aware assignment of the occupied voxels to
  * n tiny networks -- "pop an unassigned voxel with the minimum coordinate as the anchor; search s-1 nearest
@@ -188,9 +238,10 @@ typedef struct {
   float ms_mlp;
   float ms_composite;
   float ms_total;
+  uint32_t retries;          /* chunks rendered again because they outgrew the buffers, since scene creation */
 } r360_stats;
 
-/* Statistics of the last render call; synchronises the scene's stream. */
+/* Statistics of the last render call; synchronises the scene's stream (and settles the call like r360_wait). */
 r360_status r360_get_stats(r360_scene* scene, r360_stats* out);
 
 /* Debug tap for the parity tests (steps a1-a5): runs the sampler and the binning for

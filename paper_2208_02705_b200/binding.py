@@ -30,7 +30,7 @@ class Stats(C.Structure):
                 ("samples_used", C.c_uint64), ("mlp_tiles", C.c_uint64), ("chunks", C.c_uint32),
                 ("kernel_launches", C.c_uint32), ("ms_count", C.c_float), ("ms_scan", C.c_float),
                 ("ms_emit", C.c_float), ("ms_mlp", C.c_float), ("ms_composite", C.c_float),
-                ("ms_total", C.c_float)]
+                ("ms_total", C.c_float), ("retries", C.c_uint32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -65,6 +65,18 @@ def lib():
     L.r360_render_batch.argtypes = [vp, f32p, i32, i32, i32, vp, vp]
     L.r360_render_batch_host.restype = C.c_int
     L.r360_render_batch_host.argtypes = [vp, f32p, i32, i32, i32, vp, vp]
+    L.r360_render_rows.restype = C.c_int
+    L.r360_render_rows.argtypes = [vp, f32p, i32, i32, i32, i32, vp, vp]
+    for name in ("r360_wait", "r360_graph_status"):
+        getattr(L, name).restype = C.c_int
+        getattr(L, name).argtypes = [vp]
+    for name in ("r360_set_output_format", "r360_set_host_bands"):
+        getattr(L, name).restype = C.c_int
+        getattr(L, name).argtypes = [vp, i32]
+    L.r360_reserve.restype = C.c_int
+    L.r360_reserve.argtypes = [vp, C.c_uint64, C.c_double]
+    L.r360_set_graph_poses.restype = C.c_int
+    L.r360_set_graph_poses.argtypes = [vp, f32p, i32]
     L.r360_set_precision.restype = C.c_int
     L.r360_set_precision.argtypes = [vp, i32]
     L.r360_assign_subfields.restype = C.c_int
@@ -228,36 +240,86 @@ class Scene:
         import torch
         self.set_stream(torch.cuda.current_stream().cuda_stream)
 
-    def render(self, pose, W, H, out_rgb=None, out_depth=None):
-        return self.render_batch(np.asarray(pose, np.float32).reshape(1, 12), W, H, out_rgb, out_depth, _single=True)
+    def set_output_format(self, fmt):
+        """"f32" (rgb float32 x 3 + depth float32, default) or "rgb8_d16" (rgb uint8 x 3 + depth float16)."""
+        f = {"f32": 0, "rgb8_d16": 1}.get(fmt, fmt)
+        _check(lib().r360_set_output_format(self._h, f), "r360_set_output_format")
+        self._fmt = int(f)
 
-    def render_batch(self, poses, W, H, out_rgb=None, out_depth=None, _single=False):
+    def set_host_bands(self, n):
+        _check(lib().r360_set_host_bands(self._h, int(n)), "r360_set_host_bands")
+
+    def reserve(self, max_rays_per_chunk, segments_per_ray):
+        _check(lib().r360_reserve(self._h, int(max_rays_per_chunk), float(segments_per_ray)), "r360_reserve")
+
+    def wait(self):
+        """r360_wait: the outputs of the last render call are complete in stream order once this returns."""
+        _check(lib().r360_wait(self._h), "r360_wait")
+
+    def graph_status(self):
+        _check(lib().r360_graph_status(self._h), "r360_graph_status")
+
+    def set_graph_poses(self, poses):
+        poses = np.asarray(poses, np.float32)
+        keep, p = _pose_ptr(poses, poses.size // 12)
+        _check(lib().r360_set_graph_poses(self._h, p, poses.size // 12), "r360_set_graph_poses")
+
+    def _out_tensors(self, shape_px, out_rgb, out_depth):
         import torch
+        fmt = getattr(self, "_fmt", 0)
+        t_rgb, t_d = (torch.float32, torch.float32) if fmt == 0 else (torch.uint8, torch.float16)
+        n = int(np.prod(shape_px))
+        if out_rgb is None:
+            out_rgb = torch.empty((*shape_px, 3), dtype=t_rgb, device="cuda")
+        if out_depth is None:
+            out_depth = torch.empty(tuple(shape_px), dtype=t_d, device="cuda")
+        assert out_rgb.is_cuda and out_depth.is_cuda and out_rgb.is_contiguous() and out_depth.is_contiguous()
+        assert out_rgb.dtype == t_rgb and out_depth.dtype == t_d
+        assert out_rgb.numel() == n * 3 and out_depth.numel() == n
+        return out_rgb, out_depth
+
+    def render(self, pose, W, H, out_rgb=None, out_depth=None, wait=True):
+        """r360_render (+ r360_wait unless wait=False: needed before the outputs are used by other stream work)."""
+        out_rgb, out_depth = self._out_tensors((1, H, W), out_rgb, out_depth)
+        keep, p = _pose_ptr(pose, 1)
+        _check(lib().r360_render(self._h, p, W, H, out_rgb.data_ptr(), out_depth.data_ptr()), "r360_render")
+        if wait:
+            self.wait()
+        return out_rgb.view(H, W, 3), out_depth.view(H, W)
+
+    def render_batch(self, poses, W, H, out_rgb=None, out_depth=None, wait=True):
         poses = np.asarray(poses, np.float32)
         B = poses.size // 12
-        if out_rgb is None:
-            out_rgb = torch.empty((B, H, W, 3), dtype=torch.float32, device="cuda")
-        if out_depth is None:
-            out_depth = torch.empty((B, H, W), dtype=torch.float32, device="cuda")
-        assert out_rgb.is_cuda and out_depth.is_cuda and out_rgb.is_contiguous() and out_depth.is_contiguous()
-        assert out_rgb.numel() == B * H * W * 3 and out_depth.numel() == B * H * W
+        out_rgb, out_depth = self._out_tensors((B, H, W), out_rgb, out_depth)
         keep, p = _pose_ptr(poses, B)
-        if _single:
-            st = lib().r360_render(self._h, p, W, H, out_rgb.data_ptr(), out_depth.data_ptr())
-            _check(st, "r360_render")
-            return out_rgb.view(H, W, 3), out_depth.view(H, W)
         st = lib().r360_render_batch(self._h, p, B, W, H, out_rgb.data_ptr(), out_depth.data_ptr())
         _check(st, "r360_render_batch")
+        if wait:
+            self.wait()
+        return out_rgb, out_depth
+
+    def render_rows(self, pose, W, H, row0, row1, out_rgb=None, out_depth=None, wait=True):
+        """r360_render_rows: image rows [row0, row1) of one view into band-sized outputs [(row1-row0), W(, 3)]."""
+        out_rgb, out_depth = self._out_tensors((row1 - row0, W), out_rgb, out_depth)
+        keep, p = _pose_ptr(pose, 1)
+        st = lib().r360_render_rows(self._h, p, W, H, row0, row1, out_rgb.data_ptr(), out_depth.data_ptr())
+        _check(st, "r360_render_rows")
+        if wait:
+            self.wait()
         return out_rgb, out_depth
 
     def render_batch_host(self, poses, W, H, out_rgb=None, out_depth=None):
         """HOST buffers in and out (numpy, ideally pinned): the end-to-end call."""
         poses = np.asarray(poses, np.float32)
         B = poses.size // 12
+        fmt = getattr(self, "_fmt", 0)
+        t_rgb, t_d = (np.float32, np.float32) if fmt == 0 else (np.uint8, np.float16)
         if out_rgb is None:
-            out_rgb = np.empty((B, H, W, 3), np.float32)
+            out_rgb = np.empty((B, H, W, 3), t_rgb)
         if out_depth is None:
-            out_depth = np.empty((B, H, W), np.float32)
+            out_depth = np.empty((B, H, W), t_d)
+        assert out_rgb.dtype == t_rgb and out_depth.dtype == t_d
+        assert out_rgb.size == B * H * W * 3 and out_depth.size == B * H * W
         keep, p = _pose_ptr(poses, B)
         st = lib().r360_render_batch_host(self._h, p, B, W, H, out_rgb.ctypes.data, out_depth.ctypes.data)
         _check(st, "r360_render_batch_host")

@@ -158,17 +158,21 @@ void r360_scene_destroy(r360_scene* sc) {
   cudaFree(sc->buf.ray_cnt); cudaFree(sc->buf.ray_off); cudaFree(sc->buf.block_sum);
   cudaFree(sc->buf.bin_cnt); cudaFree(sc->buf.bin_start); cudaFree(sc->buf.bin_cursor);
   cudaFree(sc->buf.tile_start); cudaFree(sc->buf.totals);
+  cudaDeviceSynchronize();   // (work of the last calls may still use the buffers)
   cudaFree(sc->buf.seg_tin); cudaFree(sc->buf.seg_dt); cudaFree(sc->buf.recs); cudaFree(sc->buf.out);
   cudaFree(sc->d_dirblk);
   cudaFree(sc->buf.hit_t); cudaFree(sc->buf.hit_lab);
   cudaFree(sc->buf.bin_ovf); cudaFree(sc->buf.blk_list); cudaFree(sc->buf.blk_list_n);
   cudaFree(sc->d_pass_cnt); cudaFree(sc->buf.pass_off); cudaFree(sc->buf.st_c); cudaFree(sc->buf.st_T);
   cudaFree(sc->d_stage_rgb); cudaFree(sc->d_stage_depth);
-  if (sc->h_totals) cudaFreeHost(sc->h_totals);
+  if (sc->h_snap) cudaFreeHost(sc->h_snap);
+  if (sc->h_poses) cudaFreeHost(sc->h_poses);
   if (sc->copy_stream) cudaStreamDestroy(sc->copy_stream);
   if (sc->ev_chunk_done) cudaEventDestroy(sc->ev_chunk_done);
-  for (auto& ce : sc->events)
+  for (auto& ce : sc->events) {
     for (auto& e : ce.e) cudaEventDestroy(e);
+    cudaEventDestroy(ce.scanned);
+  }
   cudaGetLastError();
   delete sc;
 }
@@ -302,8 +306,13 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
   R360_CUDA(cudaMalloc(&sc->buf.bin_start, (size_t)(n + 1) * 4));
   R360_CUDA(cudaMalloc(&sc->buf.bin_cursor, (size_t)n * 4));
   R360_CUDA(cudaMalloc(&sc->buf.tile_start, (size_t)(n + 1) * 4));
-  R360_CUDA(cudaMalloc(&sc->buf.totals, 4 * sizeof(unsigned long long)));
-  R360_CUDA(cudaMallocHost(&sc->h_totals, 4 * sizeof(unsigned long long)));
+  R360_CUDA(cudaMalloc(&sc->buf.totals, kTotN * sizeof(unsigned long long)));
+  {
+    const size_t bytes = (size_t)r360_scene::kMaxChunks * 2 * kTotN * sizeof(unsigned long long);
+    R360_CUDA(cudaHostAlloc(&sc->h_snap, bytes, cudaHostAllocMapped));
+    std::memset(sc->h_snap, 0, bytes);
+    R360_CUDA(cudaHostGetDevicePointer(&sc->d_snap, sc->h_snap, 0));
+  }
   guard.s = nullptr;
   *out = sc;
   return R360_OK;

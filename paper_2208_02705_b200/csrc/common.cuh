@@ -38,6 +38,8 @@ __device__ __forceinline__ float seg_delta(const GridParams& g, float t_in, floa
 struct FrameParams {
   int W, H;
   long long ray0;        // first global ray of this chunk
+  long long out0;        // index of the chunk's first ray in the caller's output buffers (ray0 - first ray of the call)
+  int out_format;        // r360_output_format: 0 = rgb float[3] + depth float, 1 = rgb uint8[3] + depth binary16
   unsigned pose0;        // ray0 / (W*H)
   unsigned pix0;         // ray0 % (W*H)
   unsigned n_rays;       // rays in this chunk

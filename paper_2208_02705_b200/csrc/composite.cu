@@ -62,10 +62,11 @@ __device__ __forceinline__ void composite_half_segments(const ChunkBuffers& b, u
 // registers do not cost the K = 8 case occupancy); 0 = the general loop
 template <bool HALF, int KFAST>
 __global__ void __launch_bounds__(128)
-k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __restrict__ out_rgb,
-            float* __restrict__ out_depth, PassParams pp) {
+k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, void* __restrict__ out_rgb,
+            void* __restrict__ out_depth, PassParams pp) {
   const unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
   unsigned used = 0;
+  if (chunk_cancelled(b)) return;
   // wavefront pass: rays that finished in an earlier pass have nothing left to do
   if (r < f.n_rays && !(pp.wavefront && !pp.first && b.st_T[r] < 0.0f)) {
     const unsigned cnt = pp.wavefront ? b.pass_cnt[r] : b.ray_cnt[r];
@@ -144,21 +145,29 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, float* __res
       write_out = finished;
     }
     if (write_out) {
-      const size_t gr = (size_t)(f.ray0 + (long long)r);
-      out_rgb[gr * 3 + 0] = C0;
-      out_rgb[gr * 3 + 1] = C1;
-      out_rgb[gr * 3 + 2] = C2;
-      out_depth[gr] = D;
+      const size_t gr = (size_t)(f.out0 + (long long)r);
+      if (f.out_format == 0) {
+        float* o = reinterpret_cast<float*>(out_rgb) + gr * 3;
+        o[0] = C0; o[1] = C1; o[2] = C2;
+        reinterpret_cast<float*>(out_depth)[gr] = D;
+      } else {
+        // R360_OUT_RGB8_D16: colour rounded to the nearest of 256 levels, depth to binary16
+        uint8_t* o = reinterpret_cast<uint8_t*>(out_rgb) + gr * 3;
+        o[0] = (uint8_t)__float2int_rn(__saturatef(C0) * 255.0f);
+        o[1] = (uint8_t)__float2int_rn(__saturatef(C1) * 255.0f);
+        o[2] = (uint8_t)__float2int_rn(__saturatef(C2) * 255.0f);
+        reinterpret_cast<__half*>(out_depth)[gr] = __float2half_rn(D);
+      }
     }
   }
   // samples_used statistic
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) used += __shfl_xor_sync(0xffffffffu, used, o);
-  if ((threadIdx.x & 31) == 0 && used) atomicAdd(&b.totals[2], (unsigned long long)used);
+  if ((threadIdx.x & 31) == 0 && used) atomicAdd(&b.totals[kTotUsed], (unsigned long long)used);
 }
 
 void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
-                      float* out_rgb, float* out_depth, const PassParams& pp, bool half_samples, cudaStream_t s) {
+                      void* out_rgb, void* out_depth, const PassParams& pp, bool half_samples, cudaStream_t s) {
   const dim3 grid((f.n_rays + 127) / 128), block(128);
   if (!half_samples) k_composite<false, 0><<<grid, block, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);
   else if (g.K == 8) k_composite<true, 8><<<grid, block, 0, s>>>(g, f, b, tau, out_rgb, out_depth, pp);

@@ -44,7 +44,9 @@ struct ChunkBuffers {
   uint32_t* bin_start;   // [n+1]
   uint32_t* bin_cursor;  // [n]
   uint32_t* tile_start;  // [n+1] first MLP tile of each subfield
-  unsigned long long* totals;  // [4]: segments, tiles, samples_used (accumulated), spare
+  unsigned long long* totals;  // [kTotN] device-side counters of the current ray chunk (indices below)
+  unsigned long long* host_flags;  // mapped pinned host memory, [2]: k_scan posts {overflow flag, largest pass} of the
+                                   // chunk here, so the host learns them without a copy in the stream
   float* seg_tin;        // [G] ray-major
   float* seg_dt;         // [G] ray-major
   SegRec* recs;          // [G * kRecWords] binned by subfield (common.cuh: SegRec)
@@ -63,6 +65,26 @@ struct ChunkBuffers {
   int dir_f16;           // operand format of dirblk: 0 bfloat16, 1 binary16
 };
 
+// ChunkBuffers::totals, reset at the start of every ray chunk.  The kernels that follow k_scan size nothing on
+// the host: they read the counts from here, and they return at once when kTotOverflow is set (the chunk's
+// segments exceed the capacity of the segment buffers: the host re-renders the chunk with larger buffers, see
+// render.cu) or when kTotWaveDone is set (wavefront: every ray has finished, the remaining passes have no work).
+enum : int {
+  kTotSegs = 0,       // segments of the current pass (k_scan)
+  kTotTiles = 1,      // MLP tiles of the current pass (k_scan)
+  kTotUsed = 2,       // samples composited before early-out, summed over the chunk's passes (k_composite)
+  kTotGeo = 3,        // wavefront: occupied voxels crossed by all rays (k_count); single pass: unused
+  kTotOverflow = 4,   // sticky: a pass had more segments than seg_cap
+  kTotWaveDone = 5,   // sticky: a wavefront pass after the first had no segments
+  kTotSegSum = 6,     // segments summed over the chunk's passes
+  kTotTileSum = 7,    // tiles summed over the chunk's passes
+  kTotSegMax = 8,     // largest pass of the chunk, in segments (sizes the buffers of later frames)
+  kTotN = 16
+};
+__device__ __forceinline__ bool chunk_cancelled(const ChunkBuffers& b) {
+  return (b.totals[kTotOverflow] | b.totals[kTotWaveDone]) != 0;
+}
+
 constexpr int kSamplerThreads = 256;
 
 // Wavefronted early termination: the hits of a ray are fed to the MLP in passes
@@ -80,7 +102,10 @@ constexpr int kBlkListCap = 256;
 
 void launch_count(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
                   int n_bins, cudaStream_t s);
-void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_tile, cudaStream_t s);
+// seg_cap: capacity of the segment buffers (seg_tin, seg_dt, recs, out) in segments; later_wave_pass: a wavefront
+// pass after the first (an empty one ends the chunk)
+void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_tile, unsigned long long seg_cap,
+                 int later_wave_pass, cudaStream_t s);
 void launch_emit(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
                  int n_bins, const PassParams& pp, cudaStream_t s);
 // wavefront: segments of every ray in this pass, block-local offsets, the pass's histogram and reservations
@@ -98,7 +123,7 @@ cudaError_t launch_mlp_tc(const GridParams& g, const FrameParams& f, const Chunk
                           const SubfieldFrame* frames, int n_bins, int segs_per_tile, int n_sms,
                           cudaStream_t s);
 void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
-                      float* out_rgb, float* out_depth, const PassParams& pp, bool half_samples, cudaStream_t s);
+                      void* out_rgb, void* out_depth, const PassParams& pp, bool half_samples, cudaStream_t s);
 // debug: expand binned records into ray-major per-sample t and subfield id
 void launch_export_samples(const GridParams& g, const ChunkBuffers& b, int n_bins, unsigned n_segs,
                            float* t, int32_t* subfield, cudaStream_t s);

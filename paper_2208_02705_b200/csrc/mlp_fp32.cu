@@ -57,7 +57,8 @@ k_mlp_fp32(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, Fp32Layout
   float* sw = smem;                       // [lay.total]
   float* act = smem + lay.total;          // [WD][128], column = thread
   const int tid = threadIdx.x;
-  const unsigned total_tiles = (unsigned)b.totals[1];
+  if (chunk_cancelled(b)) return;
+  const unsigned total_tiles = (unsigned)b.totals[kTotTiles];
   const unsigned per = (total_tiles + gridDim.x - 1) / gridDim.x;
   const unsigned tile0 = blockIdx.x * per;
   const unsigned tile1 = min(total_tiles, tile0 + per);

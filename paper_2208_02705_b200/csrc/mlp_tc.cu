@@ -310,7 +310,8 @@ k_mlp_tc(GridParams g, FrameParams f, ChunkBuffers b, NetShape net, TcLayout lay
   const int grp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 7), 0);
   const int tid = threadIdx.x & (kTileRows - 1);
   const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
-  const unsigned total_tiles = (unsigned)b.totals[1];
+  if (chunk_cancelled(b)) return;                              // (before anything is allocated)
+  const unsigned total_tiles = (unsigned)b.totals[kTotTiles];
   const unsigned n_groups = gridDim.x * G;
   const unsigned per = (total_tiles + n_groups - 1) / n_groups;
   if ((unsigned)blockIdx.x * G * per >= total_tiles) return;   // whole CTA idle: nothing allocated yet

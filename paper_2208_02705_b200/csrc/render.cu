@@ -1,6 +1,18 @@
 // r360 -- render orchestration behind r360_render* (host code; all compute in the kernels).
+//
+// A call is cut into ray chunks (r360_set_chunk_rays); a chunk is 5 kernel launches (k_count, k_scan, k_emit,
+// k_mlp_*, k_composite), or one such group per pass with r360_set_wavefront.  The host never waits for the GPU
+// in the middle of a frame: the kernels behind k_scan take their counts from device memory (kernels.h: totals),
+// and the segment buffers (seg_tin, seg_dt, recs, out) are sized from a CAPACITY learnt from earlier frames
+// (largest segments-per-ray ratio seen, plus a quarter).  If a chunk has more segments than the capacity, k_scan
+// raises kTotOverflow, the chunk's remaining kernels return at once, and the host -- which finds the flag in
+// mapped pinned memory at its next call on the scene (r360_settle: r360_wait, r360_get_stats, the next render
+// ...) -- renders that chunk again with larger buffers, in stream order, before anything else.  Nothing is ever
+// truncated.  The very first chunk of a scene (no ratio known yet) and every retry run in the exact mode: the
+// host waits for k_scan and sizes the buffers from the true count.
 #include <cmath>
 #include <cstring>
+#include <new>
 
 #include "scene.h"
 
@@ -10,15 +22,25 @@ namespace {
 
 constexpr double kPi = 3.14159265358979323846;
 
+// Inside a stream capture nothing may be allocated (g_no_alloc): a buffer that is too small is R360_ERR_CAPACITY.
+thread_local bool g_no_alloc = false;
+
 template <typename T>
-r360_status grow(T*& p, size_t& cap, size_t need, size_t slack_num = 5, size_t slack_den = 4) {
+r360_status grow(T*& p, size_t& cap, size_t need) {
   if (need <= cap && p) return R360_OK;
-  if (p) { cudaFree(p); p = nullptr; }
-  size_t want = need * slack_num / slack_den + 64;
+  if (g_no_alloc) return R360_ERR_CAPACITY;
+  if (p) { cudaFree(p); p = nullptr; }           // (waits for the work that still uses it)
+  const size_t want = need + 64;
   cudaError_t e = cudaMalloc(&p, want * sizeof(T));
   if (e != cudaSuccess) { cap = 0; return r360_cuda_fail(e, "cudaMalloc(chunk buffer)"); }
   cap = want;
   return R360_OK;
+}
+
+bool capturing(cudaStream_t s) {
+  cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(s, &st) != cudaSuccess) { cudaGetLastError(); return false; }
+  return st != cudaStreamCaptureStatusNone;
 }
 
 // Reading B1/B2: pixel-centre angles and their trig in binary64 libm, rounded once to binary32.
@@ -26,7 +48,9 @@ r360_status ensure_tables(r360_scene* sc, int W, int H) {
   if (sc->d_tables && sc->tab_W == W && sc->tab_H == H && sc->tab_cam_model == sc->cam_model &&
       (sc->cam_model == 0 || std::memcmp(sc->tab_cam, sc->cam, sizeof(sc->cam)) == 0))
     return R360_OK;
-  std::vector<float> t((size_t)2 * W + 2 * H, 0.0f);
+  if (capturing(sc->stream)) return R360_ERR_CAPACITY;   // (render this image size once before capturing)
+  std::vector<float> t;
+  try { t.assign((size_t)2 * W + 2 * H, 0.0f); } catch (const std::bad_alloc&) { return R360_ERR_OOM; }
   if (sc->cam_model == 1) {
     // reading P: x_i = (i + 0.5 - cx)/fx, y_j = (j + 0.5 - cy)/fy in binary64, rounded once to binary32
     for (int i = 0; i < W; ++i) t[i] = (float)((((double)i + 0.5) - sc->cam[2]) / sc->cam[0]);
@@ -42,9 +66,10 @@ r360_status ensure_tables(r360_scene* sc, int W, int H) {
     t[(size_t)2 * W + j] = (float)std::sin(theta);
     t[(size_t)2 * W + H + j] = (float)std::cos(theta);
   }
+  // earlier frames may still be reading the old tables: cudaFree waits for the device
   if (sc->d_tables) { cudaFree(sc->d_tables); sc->d_tables = nullptr; }
   R360_CUDA(cudaMalloc(&sc->d_tables, t.size() * sizeof(float)));
-  // synchronous copy from a stack-owned vector; ordered before later work on sc->stream by a sync
+  // copy from a stack-owned vector; ordered before later work on sc->stream by a sync
   R360_CUDA(cudaMemcpyAsync(sc->d_tables, t.data(), t.size() * sizeof(float), cudaMemcpyHostToDevice, sc->stream));
   R360_CUDA(cudaStreamSynchronize(sc->stream));
   sc->tab_W = W;
@@ -57,21 +82,41 @@ r360_status ensure_tables(r360_scene* sc, int W, int H) {
 r360_status upload_poses(r360_scene* sc, const float* poses, int B) {
   for (int i = 0; i < B * 12; ++i)
     if (!std::isfinite(poses[i])) return R360_ERR_INVALID_ARG;
+  const bool cap = capturing(sc->stream);
   if (B > sc->poses_cap) {
+    if (cap) return R360_ERR_CAPACITY;
     if (sc->d_poses) { cudaFree(sc->d_poses); sc->d_poses = nullptr; }
+    if (sc->h_poses) { cudaFreeHost(sc->h_poses); sc->h_poses = nullptr; }
+    sc->poses_cap = 0;
     R360_CUDA(cudaMalloc(&sc->d_poses, (size_t)B * 12 * sizeof(float)));
+    R360_CUDA(cudaMallocHost(&sc->h_poses, (size_t)B * 12 * sizeof(float)));
     sc->poses_cap = B;
   }
-  // pageable source: the runtime stages it before returning, the caller may reuse `poses`
-  R360_CUDA(cudaMemcpyAsync(sc->d_poses, poses, (size_t)B * 12 * sizeof(float), cudaMemcpyHostToDevice, sc->stream));
+  if (cap) {
+    // inside a CUDA graph: the copy node reads the scene's pinned pose buffer at every replay, so a replay
+    // renders whatever r360_set_graph_poses put there last
+    std::memcpy(sc->h_poses, poses, (size_t)B * 12 * sizeof(float));
+    R360_CUDA(cudaMemcpyAsync(sc->d_poses, sc->h_poses, (size_t)B * 12 * sizeof(float), cudaMemcpyHostToDevice, sc->stream));
+  } else {
+    // pageable source: the runtime stages it before returning, the caller may reuse `poses`
+    R360_CUDA(cudaMemcpyAsync(sc->d_poses, poses, (size_t)B * 12 * sizeof(float), cudaMemcpyHostToDevice, sc->stream));
+  }
   return R360_OK;
 }
 
-FrameParams frame_params(const r360_scene* sc, int W, int H, long long ray0, unsigned n_rays) {
+struct ChunkJob {
+  long long ray0;        // first global ray (pose * W * H + pixel)
+  unsigned n_rays;
+  long long out0;        // index of that ray in the caller's output buffers
+};
+
+FrameParams frame_params(const r360_scene* sc, int W, int H, const ChunkJob& job) {
   FrameParams f;
-  f.W = W; f.H = H; f.ray0 = ray0; f.n_rays = n_rays;
-  f.pose0 = (unsigned)(ray0 / ((long long)W * H));
-  f.pix0 = (unsigned)(ray0 % ((long long)W * H));
+  f.W = W; f.H = H; f.ray0 = job.ray0; f.n_rays = job.n_rays;
+  f.out0 = job.out0;
+  f.out_format = sc->out_format;
+  f.pose0 = (unsigned)(job.ray0 / ((long long)W * H));
+  f.pix0 = (unsigned)(job.ray0 % ((long long)W * H));
   f.camera = sc->cam_model;
   f.poses = sc->d_poses;
   f.sin_phi = sc->d_tables;
@@ -86,169 +131,286 @@ r360_scene::ChunkEvents* chunk_events(r360_scene* sc, unsigned idx) {
     r360_scene::ChunkEvents ce;
     for (auto& e : ce.e)
       if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
-    sc->events.push_back(ce);
+    if (cudaEventCreateWithFlags(&ce.scanned, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+    try { sc->events.push_back(ce); } catch (const std::bad_alloc&) { return nullptr; }
   }
   return &sc->events[idx];
 }
 
-// Steps a1-a5 for one chunk: count, scan, (sync for the segment total), emit.  pp.wavefront: one pass of the
-// wavefronted path -- the walk (k_count) runs with the first pass only, every pass bins its own hit range.
-r360_status sample_chunk(r360_scene* sc, const FrameParams& f, r360_scene::ChunkEvents* ev,
-                         unsigned long long& n_segs, unsigned long long& n_tiles, unsigned& launches,
-                         const PassParams& pp) {
-  const int n = sc->desc.n_subfields;
-  const size_t n_blocks = (f.n_rays + kSamplerThreads - 1) / kSamplerThreads;
+size_t out_bytes_per_segment(const r360_scene* sc) {
+  // per-sample MLP outputs (sigma, r, g, b): float4 on the fp32 path, four binary16 values on the tensor paths
+  return (size_t)sc->grid_p.K * (sc->precision >= 1 ? 8 : 16);
+}
+
+// capacity of the segment buffers, in segments
+unsigned long long seg_capacity(const r360_scene* sc) {
+  size_t c = sc->seg_tin_cap;
+  if (sc->seg_dt_cap < c) c = sc->seg_dt_cap;
+  if (sc->recs_cap / kRecWords < c) c = sc->recs_cap / kRecWords;
+  const size_t oc = sc->out_cap_bytes / out_bytes_per_segment(sc);
+  if (oc < c) c = oc;
+  if (c > 0xFFFFFFFFull) c = 0xFFFFFFFFull;                   // 32-bit segment slots
+  return (unsigned long long)c;
+}
+
+// segments a chunk of n_rays rays is given room for: the largest segments-per-ray ratio seen so far + 25 %
+size_t expected_segments(const r360_scene* sc, size_t n_rays) {
+  return (size_t)(sc->segs_per_ray_max * 1.25 * (double)n_rays) + 4096;
+}
+
+r360_status grow_segment_buffers(r360_scene* sc, size_t n_segs) {
   r360_status st;
-  if ((st = grow(sc->buf.ray_cnt, sc->ray_cnt_cap, f.n_rays, 1, 1)) != R360_OK) return st;
-  if ((st = grow(sc->buf.ray_off, sc->ray_off_cap, f.n_rays, 1, 1)) != R360_OK) return st;
-  if ((st = grow(sc->buf.block_sum, sc->blocks_cap, n_blocks, 1, 1)) != R360_OK) return st;
-  if ((st = grow(sc->buf.hit_t, sc->hit_t_cap, (size_t)f.n_rays * kHitCap, 1, 1)) != R360_OK) return st;
-  if ((st = grow(sc->buf.hit_lab, sc->hit_lab_cap, (size_t)f.n_rays * kHitCap, 1, 1)) != R360_OK) return st;
+  if ((st = grow(sc->buf.seg_tin, sc->seg_tin_cap, n_segs)) != R360_OK) return st;
+  if ((st = grow(sc->buf.seg_dt, sc->seg_dt_cap, n_segs)) != R360_OK) return st;
+  if ((st = grow(sc->buf.recs, sc->recs_cap, n_segs * kRecWords)) != R360_OK) return st;
+  unsigned char* o = reinterpret_cast<unsigned char*>(sc->buf.out);
+  st = grow(o, sc->out_cap_bytes, n_segs * out_bytes_per_segment(sc));
+  sc->buf.out = reinterpret_cast<float4*>(o);
+  return st;
+}
+
+// One chunk: steps a1-a10.  exact: wait for every k_scan and size the segment buffers from its count (first
+// chunk of a scene, retries, r360_debug_samples); otherwise nothing waits for the GPU.
+// sample_only: stop behind k_emit (r360_debug_samples); n_segs_out then receives the segment count.
+r360_status run_chunk(r360_scene* sc, int W, int H, const ChunkJob& job, unsigned chunk_idx, bool exact,
+                      void* out_rgb, void* out_depth, unsigned& launches, bool sample_only = false,
+                      unsigned long long* n_segs_out = nullptr) {
+  const int n = sc->desc.n_subfields;
+  const FrameParams f = frame_params(sc, W, H, job);
+  const size_t n_blocks = (f.n_rays + kSamplerThreads - 1) / kSamplerThreads;
+  cudaStream_t s = sc->stream;
+  const bool cap = capturing(s);
+  if (chunk_idx >= r360_scene::kMaxChunks) return R360_ERR_INVALID_ARG;
+  r360_status st;
+  struct NoAlloc {                                             // nothing is allocated inside a stream capture
+    explicit NoAlloc(bool on) { g_no_alloc = on; }
+    ~NoAlloc() { g_no_alloc = false; }
+  } no_alloc(cap);
+  if ((st = grow(sc->buf.ray_cnt, sc->ray_cnt_cap, f.n_rays)) != R360_OK) return st;
+  if ((st = grow(sc->buf.ray_off, sc->ray_off_cap, f.n_rays)) != R360_OK) return st;
+  if ((st = grow(sc->buf.block_sum, sc->blocks_cap, n_blocks)) != R360_OK) return st;
+  if ((st = grow(sc->buf.hit_t, sc->hit_t_cap, (size_t)f.n_rays * kHitCap)) != R360_OK) return st;
+  if ((st = grow(sc->buf.hit_lab, sc->hit_lab_cap, (size_t)f.n_rays * kHitCap)) != R360_OK) return st;
   if (sc->precision >= 1) {            // tensor path: per-ray records (direction + packed F(d))
-    if ((st = grow(sc->d_dirblk, sc->dirblk_cap, (size_t)f.n_rays * 4, 1, 1)) != R360_OK) return st;
+    if ((st = grow(sc->d_dirblk, sc->dirblk_cap, (size_t)f.n_rays * 4)) != R360_OK) return st;
     sc->buf.dirblk = sc->d_dirblk;
     sc->buf.dir_f16 = sc->precision == 2;
   } else {
     sc->buf.dirblk = nullptr;
   }
-  cudaStream_t s = sc->stream;
-  if ((st = grow(sc->buf.blk_list, sc->blk_list_cap, n_blocks * kBlkListCap, 1, 1)) != R360_OK) return st;
-  if ((st = grow(sc->buf.blk_list_n, sc->blk_list_n_cap, n_blocks, 1, 1)) != R360_OK) return st;
+  if ((st = grow(sc->buf.blk_list, sc->blk_list_cap, n_blocks * kBlkListCap)) != R360_OK) return st;
+  if ((st = grow(sc->buf.blk_list_n, sc->blk_list_n_cap, n_blocks)) != R360_OK) return st;
   sc->buf.pass_cnt = nullptr;
-  if (pp.wavefront) {
-    if ((st = grow(sc->d_pass_cnt, sc->pass_cnt_cap, f.n_rays, 1, 1)) != R360_OK) return st;
-    if ((st = grow(sc->buf.pass_off, sc->pass_off_cap, f.n_rays, 1, 1)) != R360_OK) return st;
-    if ((st = grow(sc->buf.st_c, sc->st_c_cap, f.n_rays, 1, 1)) != R360_OK) return st;
-    if ((st = grow(sc->buf.st_T, sc->st_T_cap, f.n_rays, 1, 1)) != R360_OK) return st;
+  const bool wave = sc->wavefront && !sample_only;
+  if (wave) {
+    if ((st = grow(sc->d_pass_cnt, sc->pass_cnt_cap, f.n_rays)) != R360_OK) return st;
+    if ((st = grow(sc->buf.pass_off, sc->pass_off_cap, f.n_rays)) != R360_OK) return st;
+    if ((st = grow(sc->buf.st_c, sc->st_c_cap, f.n_rays)) != R360_OK) return st;
+    if ((st = grow(sc->buf.st_T, sc->st_T_cap, f.n_rays)) != R360_OK) return st;
     sc->buf.pass_cnt = sc->d_pass_cnt;
   }
-  R360_CUDA(cudaMemsetAsync(sc->buf.bin_cnt, 0, (size_t)n * 4, s));
-  R360_CUDA(cudaMemsetAsync(sc->buf.bin_ovf, 0, (size_t)n * 4, s));
-  if (ev) cudaEventRecord(ev->e[0], s);
-  if (!pp.wavefront || pp.first) {
-    launch_count(sc->grid_p, sc->d_grid, f, sc->buf, n, s);
+  if (!exact && (st = grow_segment_buffers(sc, expected_segments(sc, f.n_rays))) != R360_OK) return st;
+
+  r360_scene::ChunkEvents* ev = chunk_events(sc, chunk_idx);
+  if (!ev) return R360_ERR_OOM;
+  // pinned slots of this chunk: [2c] = {overflow flag, largest pass} posted by k_scan, [2c + 1] = the counters
+  unsigned long long* snap_tot = sc->h_snap + ((size_t)chunk_idx * 2 + 1) * kTotN;
+  sc->buf.host_flags = sc->d_snap + (size_t)chunk_idx * 2 * kTotN;
+  R360_CUDA(cudaMemsetAsync(sc->buf.totals, 0, kTotN * sizeof(unsigned long long), s));
+  // single pass over all hits, or the wavefront passes (kernels.h: PassParams)
+  static const uint32_t kPassEnd[5] = {2, 6, 16, (uint32_t)kHitCap, 0xFFFFFFFFu};
+  const int n_pass = wave ? 5 : 1;
+  for (int p = 0; p < n_pass; ++p) {
+    PassParams pp{};
+    if (wave) {
+      pp.wavefront = 1;
+      pp.first = p == 0;
+      pp.last = p == n_pass - 1;
+      pp.h0 = p ? kPassEnd[p - 1] : 0;
+      pp.h1 = kPassEnd[p];
+    }
+    const bool timed = p == 0 && !cap;                         // stage times: first pass only
+    R360_CUDA(cudaMemsetAsync(sc->buf.bin_cnt, 0, (size_t)n * 4, s));
+    R360_CUDA(cudaMemsetAsync(sc->buf.bin_ovf, 0, (size_t)n * 4, s));
+    if (timed) cudaEventRecord(ev->e[0], s);
+    if (!wave || pp.first) {
+      launch_count(sc->grid_p, sc->d_grid, f, sc->buf, n, s);
+      launches += 1;
+    }
+    if (wave) {
+      launch_pass_count(sc->grid_p, sc->d_grid, f, sc->buf, n, pp, s);
+      launches += 1;
+    }
+    if (timed) cudaEventRecord(ev->e[1], s);
+    launch_scan(sc->buf, (int)n_blocks, n, sc->segs_per_tile, exact ? 0xFFFFFFFFull : seg_capacity(sc),
+                wave && !pp.first, s);
+    if (timed) cudaEventRecord(ev->e[2], s);
     launches += 1;
-  }
-  if (pp.wavefront) {
-    launch_pass_count(sc->grid_p, sc->d_grid, f, sc->buf, n, pp, s);
-    launches += 1;
-  }
-  if (ev) cudaEventRecord(ev->e[1], s);
-  launch_scan(sc->buf, (int)n_blocks, n, sc->segs_per_tile, s);
-  if (ev) cudaEventRecord(ev->e[2], s);
-  launches += 1;
-  R360_CUDA(cudaGetLastError());
-  R360_CUDA(cudaMemcpyAsync(sc->h_totals, sc->buf.totals, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
-  R360_CUDA(cudaStreamSynchronize(s));
-  n_segs = sc->h_totals[0];
-  n_tiles = sc->h_totals[1];
-  if (n_segs >= (1ull << 32)) return R360_ERR_INVALID_ARG;   // chunk too large for 32-bit slots
-  if (n_segs) {
-    if ((st = grow(sc->buf.seg_tin, sc->seg_tin_cap, n_segs)) != R360_OK) return st;
-    if ((st = grow(sc->buf.seg_dt, sc->seg_dt_cap, n_segs)) != R360_OK) return st;
-    if ((st = grow(sc->buf.recs, sc->recs_cap, n_segs * kRecWords)) != R360_OK) return st;
+    R360_CUDA(cudaGetLastError());
+    if (exact) {
+      R360_CUDA(cudaMemcpyAsync(snap_tot, sc->buf.totals, kTotN * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
+      R360_CUDA(cudaStreamSynchronize(s));
+      const unsigned long long n_segs = snap_tot[kTotSegs];
+      if (snap_tot[kTotOverflow]) return R360_ERR_INVALID_ARG;   // chunk too large for 32-bit segment slots
+      if (n_segs_out) *n_segs_out = n_segs;
+      if (p > 0 && n_segs == 0) break;                         // every ray has finished
+      double ratio = (double)n_segs / (double)f.n_rays;
+      if (ratio < 1e-6) ratio = 1e-6;                          // (an empty view still ends the exact mode)
+      if (ratio > sc->segs_per_ray_max) sc->segs_per_ray_max = ratio;
+      // room for this count, and for what the asynchronous mode will ask for a chunk of this size
+      const size_t want = expected_segments(sc, f.n_rays);
+      if ((st = grow_segment_buffers(sc, want > n_segs ? want : (size_t)n_segs)) != R360_OK) return st;
+    } else if (p == n_pass - 1 && !cap) {
+      // k_scan has posted the chunk's overflow flag to mapped host memory; r360_settle waits for this event only
+      R360_CUDA(cudaEventRecord(ev->scanned, s));
+    }
     launch_emit(sc->grid_p, sc->d_grid, f, sc->buf, n, pp, s);
     launches += 1;
     R360_CUDA(cudaGetLastError());
+    if (timed) cudaEventRecord(ev->e[3], s);
+    if (sample_only) return R360_OK;
+    cudaError_t e;
+    if (sc->precision >= 1)
+      e = launch_mlp_tc(sc->grid_p, f, sc->buf, sc->net, sc->precision == 2 ? sc->d_wpack_f16 : sc->d_wpack,
+                        sc->wpack_stride, sc->precision == 2, sc->d_frames, n, sc->segs_per_tile, sc->n_sms, s);
+    else
+      e = launch_mlp_fp32(sc->grid_p, f, sc->buf, sc->net, sc->lay, sc->d_wt, sc->d_frames, n, sc->segs_per_tile,
+                          sc->n_sms, s);
+    if (e != cudaSuccess) return r360_cuda_fail(e, "launch_mlp");
+    launches += 1;
+    if (timed) cudaEventRecord(ev->e[4], s);
+    launch_composite(sc->grid_p, f, sc->buf, sc->desc.t_threshold, out_rgb, out_depth, pp, sc->precision >= 1, s);
+    launches += 1;
+    R360_CUDA(cudaGetLastError());
+    if (timed) cudaEventRecord(ev->e[5], s);
   }
-  if (ev) cudaEventRecord(ev->e[3], s);
+  // the chunk's counters for r360_get_stats
+  R360_CUDA(cudaMemcpyAsync(snap_tot, sc->buf.totals, kTotN * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
   return R360_OK;
+}
+
+void enqueue_host_copy(r360_scene* sc, const r360_scene::Pending& pd, const ChunkJob& job) {
+  const size_t rgb_px = pd.out_format == 0 ? 3 * sizeof(float) : 3, d_px = pd.out_format == 0 ? sizeof(float) : 2;
+  cudaEventRecord(sc->ev_chunk_done, sc->stream);
+  cudaStreamWaitEvent(sc->copy_stream, sc->ev_chunk_done, 0);
+  cudaMemcpyAsync((unsigned char*)pd.host_rgb + (size_t)job.out0 * rgb_px, (unsigned char*)pd.out_rgb + (size_t)job.out0 * rgb_px,
+                  (size_t)job.n_rays * rgb_px, cudaMemcpyDeviceToHost, sc->copy_stream);
+  cudaMemcpyAsync((unsigned char*)pd.host_depth + (size_t)job.out0 * d_px, (unsigned char*)pd.out_depth + (size_t)job.out0 * d_px,
+                  (size_t)job.n_rays * d_px, cudaMemcpyDeviceToHost, sc->copy_stream);
 }
 
 }  // namespace
 
-// host_rgb / host_depth (both or neither): every chunk's part of the image is copied to host memory on a second
-// stream as soon as the chunk is composited, behind the next chunk's kernels (r360_render_batch_host)
-static r360_status render_device(r360_scene* sc, const float* poses, int B, int W, int H, float* out_rgb,
-                                 float* out_depth, float* host_rgb = nullptr, float* host_depth = nullptr) {
+// The chunks enqueued by the last render call are checked: one whose segments did not fit the buffers is rendered
+// again, exactly sized, in stream order.  block = false: only as far as the GPU has got (never waits).
+r360_status r360_settle(r360_scene* sc, bool block) {
+  r360_scene::Pending& pd = sc->pending;
+  while (pd.next < pd.chunks.size()) {
+    const unsigned c = pd.next;
+    r360_scene::ChunkEvents& ev = sc->events[c];
+    if (!block) {
+      cudaError_t q = cudaEventQuery(ev.scanned);
+      if (q == cudaErrorNotReady) return R360_OK;
+      if (q != cudaSuccess) return r360_cuda_fail(q, "cudaEventQuery");
+    } else {
+      R360_CUDA(cudaEventSynchronize(ev.scanned));
+    }
+    const unsigned long long* snap = sc->h_snap + (size_t)c * 2 * kTotN;
+    const ChunkJob job{pd.chunks[c].ray0, pd.chunks[c].n_rays, pd.chunks[c].out0};
+    const double ratio = (double)snap[1] / (double)job.n_rays;           // k_scan's host_flags: {overflow, largest pass}
+    if (ratio > sc->segs_per_ray_max) sc->segs_per_ray_max = ratio;
+    pd.next = c + 1;
+    if (snap[0]) {
+      unsigned launches = 0;
+      r360_status st = run_chunk(sc, pd.W, pd.H, job, c, /*exact=*/true, pd.out_rgb, pd.out_depth, launches);
+      sc->stats.kernel_launches += launches;
+      sc->retries += 1;
+      if (st != R360_OK) { pd.chunks.clear(); pd.next = 0; return st; }
+      if (pd.host_rgb) enqueue_host_copy(sc, pd, job);
+    }
+  }
+  return R360_OK;
+}
+
+static r360_status render_device(r360_scene* sc, const float* poses, int B, int W, int H, long long ray_begin,
+                                 long long ray_end, void* out_rgb, void* out_depth, void* host_rgb = nullptr,
+                                 void* host_depth = nullptr, int host_bands = 1) {
   if (!sc || !poses || !out_rgb || !out_depth || B < 1 || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
   if ((long long)W * H >= (1ll << 30)) return R360_ERR_INVALID_ARG;
-  const long long total_rays = (long long)B * W * H;
+  if (ray_begin < 0 || ray_end > (long long)B * W * H || ray_begin >= ray_end) return R360_ERR_INVALID_ARG;
   r360_status st;
+  const bool cap = capturing(sc->stream);
+  if (!cap && (st = r360_settle(sc, true)) != R360_OK) return st;
   if ((st = ensure_tables(sc, W, H)) != R360_OK) return st;
   if ((st = upload_poses(sc, poses, B)) != R360_OK) return st;
-  cudaStream_t s = sc->stream;
-  R360_CUDA(cudaMemsetAsync(sc->buf.totals, 0, 4 * sizeof(unsigned long long), s));
+  const long long total_rays = ray_end - ray_begin;
+  long long chunk = sc->chunk_rays < 1 ? 1 : sc->chunk_rays;
+  if (chunk > (1ll << 30)) chunk = 1ll << 30;
+  // host output: a call that is a single chunk is cut into bands, so that all but the last band's copy to the host
+  // runs behind the next band's kernels
+  if (host_rgb && host_bands > 1 && total_rays <= chunk && total_rays >= 64 * 1024 * (long long)host_bands)
+    chunk = (total_rays + host_bands - 1) / host_bands;
+  const long long n_chunks = (total_rays + chunk - 1) / chunk;
+  if (n_chunks > (long long)r360_scene::kMaxChunks) return R360_ERR_INVALID_ARG;   // (raise r360_set_chunk_rays)
+  r360_scene::Pending& pd = sc->pending;
+  try {
+    pd.chunks.clear();
+    pd.chunks.reserve((size_t)n_chunks);
+  } catch (const std::bad_alloc&) { return R360_ERR_OOM; }
+  pd.next = 0;
+  pd.W = W; pd.H = H;
+  pd.out_rgb = out_rgb; pd.out_depth = out_depth; pd.host_rgb = host_rgb; pd.host_depth = host_depth;
+  pd.out_format = sc->out_format;
   r360_stats& stats = sc->stats;
   std::memset(&stats, 0, sizeof(stats));
   stats.rays = (uint64_t)total_rays;
   unsigned launches = 0, chunk_idx = 0;
-  long long chunk = sc->chunk_rays < 1 ? 1 : sc->chunk_rays;
-  if (chunk > (1ll << 30)) chunk = 1ll << 30;
-  for (long long ray0 = 0; ray0 < total_rays; ray0 += chunk, ++chunk_idx) {
-    unsigned n_rays = (unsigned)((total_rays - ray0 < chunk) ? (total_rays - ray0) : chunk);
-    FrameParams f = frame_params(sc, W, H, ray0, n_rays);
-    r360_scene::ChunkEvents* ev = chunk_events(sc, chunk_idx);
-    // single pass over all hits, or the wavefront passes (kernels.h: PassParams)
-    static const uint32_t kPassEnd[5] = {2, 6, 16, (uint32_t)kHitCap, 0xFFFFFFFFu};
-    const int n_pass = sc->wavefront ? 5 : 1;
-    for (int p = 0; p < n_pass; ++p) {
-      PassParams pp{};
-      if (sc->wavefront) {
-        pp.wavefront = 1;
-        pp.first = p == 0;
-        pp.last = p == n_pass - 1;
-        pp.h0 = p ? kPassEnd[p - 1] : 0;
-        pp.h1 = kPassEnd[p];
-      }
-      r360_scene::ChunkEvents* pev = p == 0 ? ev : nullptr;   // stage times: first pass only
-      unsigned long long n_segs = 0, n_tiles = 0;
-      if ((st = sample_chunk(sc, f, pev, n_segs, n_tiles, launches, pp)) != R360_OK) return st;
-      if (p > 0 && n_segs == 0) break;                       // every ray has finished
-      if (n_segs) {
-        // per-sample MLP outputs: K * segments float4, ray-major
-        if ((st = grow(sc->buf.out, sc->out_cap, (size_t)n_segs * sc->grid_p.K)) != R360_OK) return st;
-        cudaError_t e;
-        if (sc->precision >= 1)
-          e = launch_mlp_tc(sc->grid_p, f, sc->buf, sc->net, sc->precision == 2 ? sc->d_wpack_f16 : sc->d_wpack,
-                            sc->wpack_stride, sc->precision == 2, sc->d_frames, sc->desc.n_subfields,
-                            sc->segs_per_tile, sc->n_sms, s);
-        else
-          e = launch_mlp_fp32(sc->grid_p, f, sc->buf, sc->net, sc->lay, sc->d_wt, sc->d_frames,
-                              sc->desc.n_subfields, sc->segs_per_tile, sc->n_sms, s);
-        if (e != cudaSuccess) return r360_cuda_fail(e, "launch_mlp");
-        launches += 1;
-      }
-      if (pev) cudaEventRecord(pev->e[4], s);
-      launch_composite(sc->grid_p, f, sc->buf, sc->desc.t_threshold, out_rgb, out_depth, pp, sc->precision >= 1, s);
-      launches += 1;
-      R360_CUDA(cudaGetLastError());
-      if (pev) cudaEventRecord(pev->e[5], s);
-      stats.segments += n_segs;
-      stats.mlp_tiles += n_tiles;
+  for (long long r0 = 0; r0 < total_rays; r0 += chunk, ++chunk_idx) {
+    const ChunkJob job{ray_begin + r0, (unsigned)((total_rays - r0 < chunk) ? (total_rays - r0) : chunk), r0};
+    // the first chunk a scene ever renders sizes the buffers from its true count; everything after is asynchronous
+    const bool exact = sc->segs_per_ray_max == 0.0;
+    if (cap && exact) return R360_ERR_CAPACITY;                // (render once before capturing)
+    if ((st = run_chunk(sc, W, H, job, chunk_idx, exact, out_rgb, out_depth, launches)) != R360_OK) {
+      pd.chunks.clear();
+      pd.next = 0;
+      return st;
     }
-    if (host_rgb) {
-      R360_CUDA(cudaEventRecord(sc->ev_chunk_done, s));
-      R360_CUDA(cudaStreamWaitEvent(sc->copy_stream, sc->ev_chunk_done, 0));
-      R360_CUDA(cudaMemcpyAsync(host_rgb + (size_t)ray0 * 3, out_rgb + (size_t)ray0 * 3, (size_t)n_rays * 3 * sizeof(float),
-                                cudaMemcpyDeviceToHost, sc->copy_stream));
-      R360_CUDA(cudaMemcpyAsync(host_depth + (size_t)ray0, out_depth + (size_t)ray0, (size_t)n_rays * sizeof(float),
-                                cudaMemcpyDeviceToHost, sc->copy_stream));
-    }
+    pd.chunks.push_back({job.ray0, job.n_rays, job.out0});
+    if (exact) pd.next = chunk_idx + 1;                        // nothing to verify
+    if (host_rgb) enqueue_host_copy(sc, pd, job);
+    if (!cap && !exact && (st = r360_settle(sc, false)) != R360_OK) return st;   // earlier chunks, without waiting
   }
-  // wavefront: `segments` counts what reached the MLP; the geometric total comes from the walk
-  stats.samples_emitted = (sc->wavefront ? (uint64_t)sc->h_totals[3] : stats.segments) * (uint64_t)sc->grid_p.K;
   stats.chunks = chunk_idx;
   stats.kernel_launches = launches;
   sc->chunks_last = chunk_idx;
+  if (cap) { pd.chunks.clear(); pd.next = 0; }                 // a captured frame is checked with r360_graph_status
   return R360_OK;
 }
 
 extern "C" {
 
 r360_status r360_render_batch(r360_scene* sc, const float* poses, int32_t B, int32_t W, int32_t H,
-                              float* out_rgb, float* out_depth) {
-  return render_device(sc, poses, B, W, H, out_rgb, out_depth);
+                              void* out_rgb, void* out_depth) {
+  return render_device(sc, poses, B, W, H, 0, (long long)B * W * H, out_rgb, out_depth);
 }
 
-r360_status r360_render(r360_scene* sc, const float pose[12], int32_t W, int32_t H, float* out_rgb,
-                        float* out_depth) {
-  return render_device(sc, pose, 1, W, H, out_rgb, out_depth);
+r360_status r360_render(r360_scene* sc, const float pose[12], int32_t W, int32_t H, void* out_rgb,
+                        void* out_depth) {
+  return render_device(sc, pose, 1, W, H, 0, (long long)W * H, out_rgb, out_depth);
+}
+
+r360_status r360_render_rows(r360_scene* sc, const float pose[12], int32_t W, int32_t H, int32_t row0, int32_t row1,
+                             void* out_rgb, void* out_depth) {
+  if (W < 1 || H < 1 || row0 < 0 || row1 > H || row0 >= row1) return R360_ERR_INVALID_ARG;
+  return render_device(sc, pose, 1, W, H, (long long)row0 * W, (long long)row1 * W, out_rgb, out_depth);
 }
 
 r360_status r360_render_batch_host(r360_scene* sc, const float* poses, int32_t B, int32_t W, int32_t H,
-                                   float* out_rgb_host, float* out_depth_host) {
+                                   void* out_rgb_host, void* out_depth_host) {
   if (!sc || !poses || !out_rgb_host || !out_depth_host || B < 1 || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
+  if (capturing(sc->stream)) return R360_ERR_INVALID_ARG;
+  r360_status st;
+  if ((st = r360_settle(sc, true)) != R360_OK) return st;
   const size_t R = (size_t)B * W * H;
   if (R > sc->stage_rays_cap) {
     cudaFree(sc->d_stage_rgb); cudaFree(sc->d_stage_depth);
@@ -262,25 +424,79 @@ r360_status r360_render_batch_host(r360_scene* sc, const float* poses, int32_t B
     R360_CUDA(cudaStreamCreateWithFlags(&sc->copy_stream, cudaStreamNonBlocking));
     R360_CUDA(cudaEventCreateWithFlags(&sc->ev_chunk_done, cudaEventDisableTiming));
   }
-  r360_status st = render_device(sc, poses, B, W, H, sc->d_stage_rgb, sc->d_stage_depth, out_rgb_host, out_depth_host);
+  st = render_device(sc, poses, B, W, H, 0, (long long)R, sc->d_stage_rgb, sc->d_stage_depth, out_rgb_host,
+                     out_depth_host, sc->host_bands);
+  // a chunk that overflowed is rendered and copied again here
+  if (st == R360_OK) st = r360_settle(sc, true);
   // on an error too: no copy may still be writing the caller's buffers when this returns
-  cudaError_t e1 = cudaStreamSynchronize(sc->copy_stream), e2 = cudaStreamSynchronize(sc->stream);
+  cudaError_t e2 = cudaStreamSynchronize(sc->stream), e1 = cudaStreamSynchronize(sc->copy_stream);
+  sc->pending.host_rgb = sc->pending.host_depth = nullptr;
   if (st != R360_OK) return st;
   if (e1 != cudaSuccess) return r360_cuda_fail(e1, "cudaStreamSynchronize(copy_stream)");
   if (e2 != cudaSuccess) return r360_cuda_fail(e2, "cudaStreamSynchronize(stream)");
   return R360_OK;
 }
 
+r360_status r360_wait(r360_scene* sc) {
+  if (!sc) return R360_ERR_INVALID_ARG;
+  return r360_settle(sc, true);
+}
+
+r360_status r360_graph_status(r360_scene* sc) {
+  if (!sc) return R360_ERR_INVALID_ARG;
+  R360_CUDA(cudaStreamSynchronize(sc->stream));
+  for (unsigned c = 0; c < sc->chunks_last; ++c)
+    if (sc->h_snap[(size_t)c * 2 * kTotN]) return R360_ERR_CAPACITY;
+  return R360_OK;
+}
+
+r360_status r360_set_graph_poses(r360_scene* sc, const float* poses, int32_t B) {
+  if (!sc || !poses || B < 1 || B > sc->poses_cap || !sc->h_poses) return R360_ERR_INVALID_ARG;
+  for (int i = 0; i < B * 12; ++i)
+    if (!std::isfinite(poses[i])) return R360_ERR_INVALID_ARG;
+  std::memcpy(sc->h_poses, poses, (size_t)B * 12 * sizeof(float));
+  return R360_OK;
+}
+
+r360_status r360_reserve(r360_scene* sc, uint64_t max_rays_per_chunk, double segments_per_ray) {
+  if (!sc || max_rays_per_chunk < 1 || max_rays_per_chunk > (1ull << 30) || !(segments_per_ray > 0.0) ||
+      !std::isfinite(segments_per_ray))
+    return R360_ERR_INVALID_ARG;
+  if (capturing(sc->stream)) return R360_ERR_INVALID_ARG;
+  r360_status st;
+  if ((st = r360_settle(sc, true)) != R360_OK) return st;
+  if (segments_per_ray > sc->segs_per_ray_max) sc->segs_per_ray_max = segments_per_ray;
+  return grow_segment_buffers(sc, expected_segments(sc, (size_t)max_rays_per_chunk));
+}
+
 r360_status r360_set_precision(r360_scene* sc, int32_t mode) {
   if (!sc || mode < 0 || mode > 2) return R360_ERR_INVALID_ARG;
   if (mode == 1 && !sc->d_wpack) return R360_ERR_INVALID_ARG;
   if (mode == 2 && !sc->d_wpack_f16) return R360_ERR_INVALID_ARG;
+  r360_status st;
+  if ((st = r360_settle(sc, true)) != R360_OK) return st;
   sc->precision = mode;
+  return R360_OK;
+}
+
+r360_status r360_set_output_format(r360_scene* sc, int32_t format) {
+  if (!sc || (format != R360_OUT_F32 && format != R360_OUT_RGB8_D16)) return R360_ERR_INVALID_ARG;
+  r360_status st;
+  if ((st = r360_settle(sc, true)) != R360_OK) return st;
+  sc->out_format = format;
+  return R360_OK;
+}
+
+r360_status r360_set_host_bands(r360_scene* sc, int32_t bands) {
+  if (!sc || bands < 1 || bands > 64) return R360_ERR_INVALID_ARG;
+  sc->host_bands = bands;
   return R360_OK;
 }
 
 r360_status r360_set_wavefront(r360_scene* sc, int32_t enable) {
   if (!sc || (enable != 0 && enable != 1)) return R360_ERR_INVALID_ARG;
+  r360_status st;
+  if ((st = r360_settle(sc, true)) != R360_OK) return st;
   sc->wavefront = enable;
   return R360_OK;
 }
@@ -290,6 +506,8 @@ r360_status r360_set_camera(r360_scene* sc, int32_t model, double fx, double fy,
   if (model == 1 && !(fx > 0.0 && fy > 0.0 && std::isfinite(fx) && std::isfinite(fy) && std::isfinite(cx) &&
                       std::isfinite(cy)))
     return R360_ERR_INVALID_ARG;
+  r360_status st;
+  if ((st = r360_settle(sc, true)) != R360_OK) return st;
   sc->cam_model = model;
   sc->cam[0] = fx; sc->cam[1] = fy; sc->cam[2] = cx; sc->cam[3] = cy;
   return R360_OK;
@@ -297,6 +515,12 @@ r360_status r360_set_camera(r360_scene* sc, int32_t model, double fx, double fy,
 
 r360_status r360_set_stream(r360_scene* sc, void* stream) {
   if (!sc) return R360_ERR_INVALID_ARG;
+  r360_status st;
+  if ((st = r360_settle(sc, true)) != R360_OK) return st;
+  if ((cudaStream_t)stream != sc->stream) {
+    // work of earlier calls on the old stream shares the scene's buffers with what follows on the new one
+    R360_CUDA(cudaStreamSynchronize(sc->stream));
+  }
   sc->stream = (cudaStream_t)stream;
   return R360_OK;
 }
@@ -309,22 +533,27 @@ r360_status r360_set_chunk_rays(r360_scene* sc, int64_t max_rays) {
 
 r360_status r360_get_stats(r360_scene* sc, r360_stats* out) {
   if (!sc || !out) return R360_ERR_INVALID_ARG;
+  r360_status rs;
+  if ((rs = r360_settle(sc, true)) != R360_OK) return rs;
   R360_CUDA(cudaStreamSynchronize(sc->stream));
   r360_stats& st = sc->stats;
   st.ms_count = st.ms_scan = st.ms_emit = st.ms_mlp = st.ms_composite = st.ms_total = 0.f;
+  st.segments = st.mlp_tiles = st.samples_used = st.samples_emitted = 0;
   for (unsigned c = 0; c < sc->chunks_last && c < sc->events.size(); ++c) {
     float ms[5] = {0, 0, 0, 0, 0};
     for (int i = 0; i < 5; ++i)
       if (cudaEventElapsedTime(&ms[i], sc->events[c].e[i], sc->events[c].e[i + 1]) != cudaSuccess) ms[i] = 0.f;
     st.ms_count += ms[0]; st.ms_scan += ms[1]; st.ms_emit += ms[2]; st.ms_mlp += ms[3]; st.ms_composite += ms[4];
+    const unsigned long long* snap = sc->h_snap + ((size_t)c * 2 + 1) * kTotN;
+    st.segments += snap[kTotSegSum];
+    st.mlp_tiles += snap[kTotTileSum];
+    st.samples_used += snap[kTotUsed];
+    // wavefront: `segments` counts what reached the MLP; the geometric total comes from the walk
+    st.samples_emitted += (sc->wavefront ? snap[kTotGeo] : snap[kTotSegSum]) * (uint64_t)sc->grid_p.K;
   }
   cudaGetLastError();
   st.ms_total = st.ms_count + st.ms_scan + st.ms_emit + st.ms_mlp + st.ms_composite;
-  if (sc->chunks_last) {
-    unsigned long long used = 0;
-    R360_CUDA(cudaMemcpy(&used, sc->buf.totals + 2, sizeof(used), cudaMemcpyDeviceToHost));
-    st.samples_used = used;
-  }
+  st.retries = sc->retries;
   *out = st;
   return R360_OK;
 }
@@ -333,15 +562,19 @@ r360_status r360_debug_samples(r360_scene* sc, const float pose[12], int32_t W, 
                                uint32_t* offsets, float* t, int32_t* subfield, uint64_t cap, uint64_t* total) {
   if (!sc || !pose || !counts || !offsets || !total || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
   if ((long long)W * H >= (1ll << 30)) return R360_ERR_INVALID_ARG;
+  if (capturing(sc->stream)) return R360_ERR_INVALID_ARG;
   r360_status st;
+  if ((st = r360_settle(sc, true)) != R360_OK) return st;
   if ((st = ensure_tables(sc, W, H)) != R360_OK) return st;
   if ((st = upload_poses(sc, pose, 1)) != R360_OK) return st;
-  FrameParams f = frame_params(sc, W, H, 0, (unsigned)((long long)W * H));
-  unsigned long long n_segs = 0, n_tiles = 0;
+  const ChunkJob job{0, (unsigned)((long long)W * H), 0};
+  unsigned long long n_segs = 0;
   unsigned launches = 0;
-  if ((st = sample_chunk(sc, f, nullptr, n_segs, n_tiles, launches, PassParams{})) != R360_OK) return st;
+  if ((st = run_chunk(sc, W, H, job, 0, /*exact=*/true, nullptr, nullptr, launches, /*sample_only=*/true, &n_segs)) != R360_OK)
+    return st;
+  sc->chunks_last = 0;
   *total = n_segs * (uint64_t)sc->grid_p.K;
-  launch_export_counts(sc->buf, f.n_rays, sc->grid_p.K, counts, offsets, sc->stream);
+  launch_export_counts(sc->buf, job.n_rays, sc->grid_p.K, counts, offsets, sc->stream);
   R360_CUDA(cudaGetLastError());
   if (*total > cap) { cudaStreamSynchronize(sc->stream); return R360_ERR_CAPACITY; }
   if (n_segs) {

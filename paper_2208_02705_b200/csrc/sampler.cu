@@ -138,7 +138,7 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
   }
   if (threadIdx.x == 0) b.block_sum[blockIdx.x] = total;
   if (b.pass_cnt) {
-    if (threadIdx.x == 0 && total) atomicAdd(&b.totals[3], (unsigned long long)total);   // geometric segments
+    if (threadIdx.x == 0 && total) atomicAdd(&b.totals[kTotGeo], (unsigned long long)total);   // geometric segments
     return;
   }
   if (use_smem_hist) {
@@ -193,11 +193,22 @@ __device__ uint64_t scan_array(const uint32_t* in, uint32_t* out, int m, uint32_
 }
 
 __global__ void __launch_bounds__(1024)
-k_scan(ChunkBuffers b, int n_blocks, int n_bins, int segs_per_tile) {
+k_scan(ChunkBuffers b, int n_blocks, int n_bins, int segs_per_tile, unsigned long long seg_cap, int later_wave_pass) {
   __shared__ uint32_t sm[34];
+  if (later_wave_pass && chunk_cancelled(b)) return;       // an earlier pass overflowed or ended the chunk
   if (blockIdx.x == 0) {
     uint64_t tot = scan_array(b.block_sum, b.block_sum, n_blocks, sm, 0, nullptr);
-    if (threadIdx.x == 0) b.totals[0] = tot;
+    if (threadIdx.x == 0) {
+      // one thread, stream order: plain read-modify-writes
+      b.totals[kTotSegs] = tot;
+      b.totals[kTotSegSum] += tot;
+      if (tot > b.totals[kTotSegMax]) b.totals[kTotSegMax] = tot;
+      if (tot > seg_cap) b.totals[kTotOverflow] = 1;
+      if (later_wave_pass && tot == 0) b.totals[kTotWaveDone] = 1;
+      b.host_flags[0] = b.totals[kTotOverflow];
+      b.host_flags[1] = b.totals[kTotSegMax];
+      __threadfence_system();
+    }
   } else {
     // a bin = [segments reserved by blocks | the rest, placed through the global cursor]
     for (int k = threadIdx.x; k < n_bins; k += blockDim.x) {
@@ -212,7 +223,8 @@ k_scan(ChunkBuffers b, int n_blocks, int n_bins, int segs_per_tile) {
     if (threadIdx.x == 0) {
       b.tile_start[n_bins] = (uint32_t)tiles;
       b.bin_start[n_bins] = (uint32_t)segs;
-      b.totals[1] = tiles;
+      b.totals[kTotTiles] = tiles;
+      b.totals[kTotTileSum] += tiles;
     }
   }
 }
@@ -227,6 +239,7 @@ k_pass_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, Chu
              int use_smem_hist, PassParams pp) {
   extern __shared__ uint32_t hist[];
   __shared__ uint32_t warp_sums[33];
+  if (chunk_cancelled(b)) return;
   if (use_smem_hist) {
     for (int k = threadIdx.x; k < n_bins; k += blockDim.x) hist[k] = 0;
     __syncthreads();
@@ -288,6 +301,7 @@ __global__ void __launch_bounds__(kSamplerThreads)
 k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuffers b, int n_bins,
        int use_smem_cursor, PassParams pp) {
   extern __shared__ uint32_t cur[];      // [n_bins] when use_smem_cursor: next position of this block in each bin
+  if (chunk_cancelled(b)) return;
   if (use_smem_cursor) load_reservations(b, cur, n_bins);
   const unsigned r = blockIdx.x * blockDim.x + threadIdx.x;
   const bool valid = r < f.n_rays;
@@ -411,8 +425,9 @@ void launch_count(const GridParams& g, const uint16_t* grid, const FrameParams& 
   k_count<<<blocks, kSamplerThreads, smem, s>>>(g, grid, f, b, n_bins, use_smem);
 }
 
-void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_tile, cudaStream_t s) {
-  k_scan<<<2, 1024, 0, s>>>(b, n_blocks, n_bins, segs_per_tile);
+void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_tile, unsigned long long seg_cap,
+                 int later_wave_pass, cudaStream_t s) {
+  k_scan<<<2, 1024, 0, s>>>(b, n_blocks, n_bins, segs_per_tile, seg_cap, later_wave_pass);
 }
 
 void launch_emit(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,

@@ -29,13 +29,20 @@ struct r360_scene {
   int tab_cam_model = -1;
   double tab_cam[4] = {0, 0, 0, 0};
   float* d_poses = nullptr;
+  float* h_poses = nullptr;                 // pinned; source of the pose copy inside a captured CUDA graph
   int poses_cap = 0;
   // chunk buffers and capacities
   r360::ChunkBuffers buf{};
   size_t ray_cnt_cap = 0, ray_off_cap = 0, blocks_cap = 0;
-  size_t seg_tin_cap = 0, seg_dt_cap = 0, recs_cap = 0, out_cap = 0, dirblk_cap = 0, hit_t_cap = 0, hit_lab_cap = 0, blk_list_cap = 0, blk_list_n_cap = 0;
+  size_t seg_tin_cap = 0, seg_dt_cap = 0, recs_cap = 0, out_cap_bytes = 0, dirblk_cap = 0, hit_t_cap = 0, hit_lab_cap = 0, blk_list_cap = 0, blk_list_n_cap = 0;
   uint4* d_dirblk = nullptr;                // owned; buf.dirblk points here only while the tensor path is selected
-  unsigned long long* h_totals = nullptr;   // pinned [4]
+  // pinned, mapped snapshots of the device counters, kMaxChunks x 2 x kTotN: [2c] = what k_scan posts for chunk c
+  // (overflow flag, largest pass), [2c + 1] = the counters at the end of the chunk (statistics)
+  static constexpr unsigned kMaxChunks = 4096;
+  unsigned long long* h_snap = nullptr;
+  unsigned long long* d_snap = nullptr;     // the same memory as the device sees it
+  double segs_per_ray_max = 0.0;            // largest segments-per-ray ratio of any chunk pass so far: sizes the buffers
+  unsigned retries = 0;                     // chunks rendered again because their segments exceeded the capacity
   // D2H staging for r360_render_batch_host
   float* d_stage_rgb = nullptr;
   float* d_stage_depth = nullptr;
@@ -45,16 +52,29 @@ struct r360_scene {
   // configuration
   cudaStream_t stream = nullptr;
   int precision = 0;                        // 0 fp32 ALUs, 1 tensor cores bfloat16, 2 tensor cores binary16
+  int out_format = 0;                       // r360_output_format
+  int host_bands = 4;                       // r360_render_batch_host cuts a single-chunk call into this many bands
   int wavefront = 0;                        // r360_set_wavefront: feed the MLP in passes, retire finished rays between them
   uint32_t* d_pass_cnt = nullptr;           // owned; buf.pass_cnt points here only during wavefront passes
   size_t pass_cnt_cap = 0, pass_off_cap = 0, st_c_cap = 0, st_T_cap = 0;
   long long chunk_rays = 4ll << 20;
   // statistics of the last call
-  struct ChunkEvents { cudaEvent_t e[6]; };
+  struct ChunkEvents { cudaEvent_t e[6]; cudaEvent_t scanned; };
   std::vector<ChunkEvents> events;   // pool, one set per chunk
   unsigned chunks_last = 0;
+  // the chunks enqueued by the last render call, until r360_settle has seen their overflow flags
+  struct PendingChunk { long long ray0; unsigned n_rays; long long out0; };
+  struct Pending {
+    std::vector<PendingChunk> chunks;
+    unsigned next = 0;                      // first chunk not yet verified
+    int W = 0, H = 0, out_format = 0;
+    void *out_rgb = nullptr, *out_depth = nullptr, *host_rgb = nullptr, *host_depth = nullptr;
+  } pending;
   r360_stats stats{};
 };
+
+// render.cu: verify the chunks of the last render call, re-render what overflowed (block: wait for their k_scan)
+r360_status r360_settle(r360_scene* sc, bool block);
 
 // records the CUDA error text for r360_last_cuda_error() and maps it to a status
 r360_status r360_cuda_fail(cudaError_t e, const char* what);

@@ -8,7 +8,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from paper_2208_02705_b200.shard import gather_rows, rank_pose, row_band
+from paper_2208_02705_b200.shard import gather_rows, rank_pose, render_sharded, row_band, stereo_poses
 
 
 def _free_port():
@@ -27,6 +27,20 @@ def _worker(rank, world, port, H, W, q):
     rows = torch.arange(r0, r1, dtype=torch.float32)[:, None, None]
     band = rows * 1000 + torch.arange(W, dtype=torch.float32)[None, :, None] + torch.tensor([0.0, 0.25, 0.5])
     full = gather_rows(band, H, rank, world, dist)
+
+    # the function bench.py --scaling strong calls, with a stand-in for Scene.render_rows that writes the same
+    # synthetic pixels (the render itself needs a GPU): every rank must end up with the whole frame
+    def fake_render_rows(pose, W_, H_, row0, row1, out_rgb, out_depth):
+        rr = torch.arange(row0, row1, dtype=torch.float32)[:, None]
+        cc = torch.arange(W_, dtype=torch.float32)[None, :]
+        out_rgb.copy_((rr * 1000 + cc)[:, :, None] + torch.tensor([0.0, 0.25, 0.5]))
+        out_depth.copy_(rr * 7 + cc)
+    full_rgb = torch.full((H, W, 3), -1.0)
+    full_d = torch.full((H, W), -1.0)
+    rows = render_sharded(fake_render_rows, None, W, H, rank, world, dist, full_rgb, full_d)
+    assert rows == (r0, r1)
+    assert torch.equal(full_rgb, full)
+    assert torch.equal(full_d, torch.arange(H, dtype=torch.float32)[:, None] * 7 + torch.arange(W, dtype=torch.float32)[None, :])
     # max-over-ranks timing reduction used by bench.py
     t = torch.tensor([float(rank + 1)], dtype=torch.float64)
     dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -55,8 +69,20 @@ def test_rank_pose_is_a_yaw_about_world_up():
     assert np.allclose(r[:, 1], [0, 0, -1], atol=1e-6)      # camera down stays world -z
 
 
-def test_two_gloo_ranks_gather_a_ragged_image():
-    world, H, W = 2, 33, 8
+def test_stereo_poses_are_one_eye_distance_apart_along_camera_x():
+    pose = np.array([0, 0, 1, 1.5, -1, 0, 0, -2.5, 0, -1, 0, 0.25], np.float32)    # camera x = world -y
+    pair = stereo_poses(pose, 0.065).reshape(2, 3, 4)
+    assert np.array_equal(pair[0][:, :3], pose.reshape(3, 4)[:, :3]) and np.array_equal(pair[1][:, :3], pair[0][:, :3])
+    assert np.allclose(pair[1][:, 3] - pair[0][:, 3], [0, -0.065, 0], atol=1e-7)
+    assert np.allclose(0.5 * (pair[0][:, 3] + pair[1][:, 3]), [1.5, -2.5, 0.25], atol=1e-7)
+
+
+import pytest
+
+
+@pytest.mark.parametrize("H", [33, 32])
+def test_two_gloo_ranks_gather_a_ragged_image(H):
+    world, W = 2, 8
     port = _free_port()
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
