@@ -3,17 +3,20 @@
 equirect render of config 3 (multi-room floor, ~1k subfields); MLP samples/s and roofline fraction.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
-                  [--precision auto|fp32|bf16]
+                  [--precision auto|fp32|bf16|f16] [--scaling weak|strong]
 
 A step = one whole pass of the hot path (ray generation, occupancy walk, binning, grouped tiny
 MLP, compositing) over one frame of synthetic input (scenegen, seeded).
-N > 1 (torchrun): every rank renders a whole frame of its own pose of the replicated scene -- rays
-are independent, no data-path collective; value = total rays of all ranks / max-over-ranks time.
+N > 1 (torchrun), --scaling weak (default): every rank renders a whole frame of its own pose of the replicated
+scene -- rays are independent, no data-path collective; value = total rays of all ranks / max-over-ranks time.
+--scaling strong: ONE frame, each rank renders its band of image rows (r360_render_rows) and the bands are
+all-gathered with NCCL (paper_2208_02705_b200.shard.render_sharded); value = rays of the frame / that time.
 --impl reference times the CPU oracle (oracle/, as it stands) on a bounded sample of the workload.
 """
 import argparse
 import json
 import os
+import statistics
 import subprocess
 import sys
 import threading
@@ -25,12 +28,10 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-FLOP_PER_SAMPLE = {(32, 2): 12160, (32, 3): 14208, (64, 3): 44800}   # algorithmic, unpadded, no biases
-# FP32 ALU peak (bound "alu"): 148 SMs x 128 FMA lanes x 2 FLOP x 1.965 GHz (B200_PROFILING.md clocks)
-ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-
 
 def flop_per_sample(width, n_hidden, pe_p=63, pe_d=27):
+    """Algorithmic FLOP of one MLP query: the unpadded contraction of the paper's network,
+    biases and positional encoding excluded.  12 160 / 14 208 / 44 800 for (32,2) / (32,3) / (64,3)."""
     macs = pe_p * width + (n_hidden - 1) * width * width + width + width * width + (width + pe_d) * width + 3 * width
     return 2 * macs
 
@@ -42,8 +43,8 @@ def executed_flop_per_sample(width, n_hidden, pe_p=63, pe_d=27):
 
 
 def ncu_traffic(kernel):
-    """DRAM bytes (read + write) of one launch of `kernel` on this workload, from the committed ncu --set full
-    capture (profiles/traffic.json, written by hand from the capture named there); None if not recorded."""
+    """DRAM bytes (read + write) of one launch of `kernel` on config 3 / bf16, from the committed ncu --set full
+    capture (profiles/traffic.json names the capture and the CSV rows it was read from); None if not recorded."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     try:
         return json.load(open(p)).get(kernel)
@@ -56,58 +57,90 @@ def measured_peaks():
     if os.path.exists(p):
         d = json.load(open(p))
         return dict(hbm=d["hbm_gbs"], bf16=d["bf16_tflops"], bf16_sustained=d["bf16_tflops_sustained"],
-                    source="measured")
-    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, source="fallback")
+                    source="MEASURED_PEAKS.json")
+    # B200_PROFILING.md's stated fallback when the driver has not written the file
+    return dict(hbm=6650.0, bf16=1590.0, bf16_sustained=1400.0, source="B200_PROFILING.md fallback")
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
-         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
-         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    """SM clock and throttle reasons DURING the timed region: NVML polled every 2 ms from a thread (nvidia-smi -lms
+    as the fallback), so that even a 40 ms region has well over five samples."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+               0x80: "hw_power_brake_slowdown"}
 
     def __init__(self, gpu_index):
         self.idx = gpu_index
-        self.rows = []
-        self.proc = None
+        self.sm, self.power = [], []
+        self.mask = 0
+        self.sm_max = None
+        self.stop_flag = False
+        self.thread = None
+        self.how = None
+
+    def _poll_nvml(self, nv, h):
+        while not self.stop_flag:
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                self.mask |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(h))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(h) / 1e3)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def _poll_smi(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        inv = {v: k for k, v in self.REASONS.items()}
+        for line in self.proc.stdout:
+            r = [x.strip() for x in line.split(",")]
+            try:
+                self.sm.append(float(r[0])); self.sm_max = float(r[1]); self.power.append(float(r[2]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    self.mask |= inv[n]
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100", "-i", str(self.idx)], stdout=subprocess.PIPE,
-                                         stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True)
-            self.t.start()
+            import pynvml as nv
+            nv.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            idx = int(vis.split(",")[self.idx]) if vis and vis.split(",")[self.idx].isdigit() else self.idx
+            h = nv.nvmlDeviceGetHandleByIndex(idx)
+            self.sm_max = float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            self.how = "nvml, 2 ms"
+            self.thread = threading.Thread(target=self._poll_nvml, args=(nv, h), daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            pass
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "--query-gpu=clocks.sm,clocks.max.sm,power.draw,"
+                                          "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+                                          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap",
+                                          "--format=csv,noheader,nounits", "-lms", "20", "-i", str(self.idx)],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.how = "nvidia-smi -lms 20"
+            self.thread = threading.Thread(target=self._poll_smi, daemon=True)
+            self.thread.start()
         except OSError:
-            self.proc = None
-
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append([x.strip() for x in line.split(",")])
+            self.how = None
 
     def stop(self):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=2)
-        except subprocess.TimeoutExpired:
-            self.proc.kill()
-        sm, mx, reasons = [], [], set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for r in self.rows:
-            if len(r) < 9:
-                continue
-            try:
-                sm.append(float(r[1])); mx.append(float(r[2]))
-            except ValueError:
-                continue
-            for n, v in zip(names, r[5:9]):
-                if v.lower().startswith("active"):
-                    reasons.add(n)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+        if self.how is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "samples": 0, "reasons": ["no NVML / nvidia-smi"]}
+        self.stop_flag = True
+        if self.how.startswith("nvidia-smi"):
+            time.sleep(0.05)
+            self.proc.terminate()
+        self.thread.join(timeout=2)
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.sm_max,
+                "sm_mhz_min": min(self.sm) if self.sm else None, "samples": len(self.sm),
+                "power_w_max": max(self.power) if self.power else None,
+                "reasons": sorted(n for b, n in self.REASONS.items() if self.mask & b), "how": self.how}
 
 
 def oracle_sample(sc, row_stride):
@@ -128,6 +161,15 @@ def oracle_sample(sc, row_stride):
                        f"{n_samples} MLP samples), wall clock")
 
 
+def workload_config(sc, args):
+    """The same dictionary in both arms (ours / reference): what is rendered, not how."""
+    return {"workload": f"BASELINE.json configs[{args.config - 1}] '{sc.name}': {sc.W}x{sc.H} equirect, "
+                        f"grid {sc.dims[0]}x{sc.dims[1]}x{sc.dims[2]}, {sc.n_subfields} subfields, "
+                        f"MLP {sc.n_hidden}x{sc.hidden_width}, K={sc.samples_per_voxel}",
+            "image": [sc.W, sc.H], "poses_per_step": 1, "n_subfields": sc.n_subfields, "seed": args.config - 1,
+            "l2": "explicit L2 flush (512 MiB memset) between timed iterations, outside the CUDA events"}
+
+
 def run_reference(args):
     """--impl reference: the oracle on this box's host cores; rank 0 only."""
     if int(os.environ.get("RANK", "0")) != 0:
@@ -146,8 +188,9 @@ def run_reference(args):
     ms = 1e3 * sum(v["seconds"] for v in vals) / len(vals)
     line = {"impl": "reference", "metric": "rays_per_second_equirect_render", "value": rays_s, "unit": "rays/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(sc, args, "oracle (geometry f32, field+compositing f64)"),
+            "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(sc, args),
+            "precision": "oracle (geometry f32, field + compositing f64)",
             "cpu_baseline": {"value": rays_s, "unit": "rays/s", "cores": vals[0]["cores"], "kind": "oracle",
                              "sample": vals[0]["sample"]},
             "e2e": {"value": rays_s, "unit": "rays/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -155,36 +198,76 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
-def workload_config(sc, args, precision):
-    return {"workload": f"BASELINE.json configs[{args.config - 1}] '{sc.name}': {sc.W}x{sc.H} equirect, "
-                        f"grid {sc.dims[0]}x{sc.dims[1]}x{sc.dims[2]}, {sc.n_subfields} subfields, "
-                        f"MLP {sc.n_hidden}x{sc.hidden_width}, K={sc.samples_per_voxel}",
-            "image": [sc.W, sc.H], "poses_per_step": 1, "n_subfields": sc.n_subfields,
-            "precision": precision, "seed": args.config - 1,
-            "l2": "explicit L2 flush (512 MiB memset) between timed iterations, outside the CUDA events"}
+def mlp_roofline(sc, precision, samples, ms_mlp, peaks, alu_peak):
+    """Roofline entry of the MLP kernel of one launch set: algorithmic FLOP / device time."""
+    fl = flop_per_sample(sc.hidden_width, sc.n_hidden)
+    ach = samples * fl / (ms_mlp * 1e-3) / 1e12 if ms_mlp > 0 else 0.0
+    if precision == "fp32":
+        return {"bound": "alu", "kernel": f"k_mlp_fp32<{sc.hidden_width}>", "achieved": ach, "peak": alu_peak["tflops"],
+                "unit": "TFLOP/s", "frac": ach / alu_peak["tflops"] if alu_peak["tflops"] else None, "traffic": None,
+                "peak_source": alu_peak["source"], "flop_per_sample": fl, "samples_per_launch": int(samples),
+                "ms_per_launch": ms_mlp}
+    ex = executed_flop_per_sample(sc.hidden_width, sc.n_hidden)
+    ach_ex = samples * ex / (ms_mlp * 1e-3) / 1e12 if ms_mlp > 0 else 0.0
+    return {"bound": "tensor", "kernel": f"k_mlp_tc<{sc.hidden_width}, {'f16' if precision == 'f16' else 'bf16'}>",
+            "achieved": ach, "peak": peaks["bf16"], "unit": "TFLOP/s", "frac": ach / peaks["bf16"], "traffic": None,
+            "peak_source": peaks["source"] + ": cuBLAS bf16 burst figure (the kernel runs at the full SM clock inside "
+                                             "a 2 ms step; binary16 operands have the same nominal rate)",
+            "frac_of_sustained": ach / peaks["bf16_sustained"], "peak_sustained": peaks["bf16_sustained"],
+            "flop_per_sample": fl,
+            # what the kernel executes after folding the feature layer into the colour layer (unpadded):
+            "executed_flop_per_sample": ex, "executed_achieved": ach_ex, "executed_frac": ach_ex / peaks["bf16"],
+            "samples_per_launch": int(samples), "ms_per_launch": ms_mlp}
 
 
-def time_config(r360, config, precision, steps=5, warmup=3, pinhole=None):
-    """Short device-timed run of another BASELINE.json config (all its poses in one batch call).
-    pinhole = (W, H, f): the same scene through the roaming (perspective) view instead of the panorama."""
+def hbm_stage_table(sc, precision, W, H, B, segs, stage_med, peaks, with_traffic):
+    """The memory-side stages against the measured HBM copy bandwidth: algorithmic bytes."""
+    rays, Kk = W * H * B, sc.samples_per_voxel
+    tensor = precision != "fp32"
+    stage_bytes = {
+        "k_count": rays * 8 + segs * 10 + (rays * 64 if tensor else 0),
+        "k_emit": rays * 8 + segs * 10 + segs * (40 if tensor else 24),
+        "k_composite": segs * Kk * (8 if tensor else 16) + segs * 8 + rays * 24,   # tensor path: binary16 x4 per sample
+    }
+    stage_key = {"k_count": "ms_count", "k_emit": "ms_emit", "k_composite": "ms_composite"}
+    out = {}
+    for kname, nbytes in stage_bytes.items():
+        ms_k = stage_med[stage_key[kname]]
+        gbs = nbytes / (ms_k * 1e-3) / 1e9 if ms_k > 0 else 0.0
+        out[kname] = {"algorithmic_bytes": int(nbytes), "ms": ms_k, "achieved_gbs": gbs,
+                      "frac_of_hbm_peak": gbs / peaks["hbm"], "traffic": ncu_traffic(kname) if with_traffic else None}
+    return out
+
+
+STAGES = ("ms_count", "ms_scan", "ms_emit", "ms_mlp", "ms_composite")
+
+
+def time_config(r360, config, precision, peaks, alu_peak, steps=5, warmup=3, pinhole=None, stereo=False):
+    """Short device-timed run of another BASELINE.json config (all its poses in one batch call), with its stage
+    times.  pinhole = (W, H, f): the same scene through the roaming (perspective) view instead of the panorama.
+    stereo: a stereoscopic pair (two eyes 65 mm apart) in one batch call instead of the config's poses."""
     import torch
     from scenegen import make_scene
     sc = make_scene(config)
     scene = r360.scene_from(sc)
     scene.set_precision(precision)
     scene.use_current_torch_stream()
-    B, W, H = len(sc.poses), sc.W, sc.H
+    W, H = sc.W, sc.H
     if pinhole:
         W, H, f = pinhole
         scene.set_camera("pinhole", f, f, W / 2.0, H / 2.0)
     poses = np.ascontiguousarray(np.stack([np.asarray(p, np.float32) for p in sc.poses]))
+    if stereo:
+        from paper_2208_02705_b200.shard import stereo_poses
+        poses = stereo_poses(sc.poses[0], 0.065)
+    B = len(poses)
     rgb = torch.empty((B, H, W, 3), dtype=torch.float32, device="cuda")
     depth = torch.empty((B, H, W), dtype=torch.float32, device="cuda")
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
     for _ in range(warmup):
         scene.render_batch(poses, W, H, rgb, depth)
     torch.cuda.synchronize()
-    ms, ms_mlp = 0.0, 0.0
+    ms, stage = [], {k: [] for k in STAGES}
     for _ in range(steps):
         flush.zero_()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -192,21 +275,20 @@ def time_config(r360, config, precision, steps=5, warmup=3, pinhole=None):
         scene.render_batch(poses, W, H, rgb, depth)
         e1.record()
         st = scene.stats()
-        ms += e0.elapsed_time(e1)
-        ms_mlp += st.ms_mlp
-    ms /= steps
-    ms_mlp /= steps
-    fl = flop_per_sample(sc.hidden_width, sc.n_hidden)
-    peaks = measured_peaks()
-    out = {"config": config, "name": sc.name + (" (pinhole view)" if pinhole else ""), "image": [W, H], "poses": B, "n_subfields": sc.n_subfields,
-           "mlp": [sc.n_hidden, sc.hidden_width], "K": sc.samples_per_voxel, "precision": precision,
-           "ms_per_step": ms, "rays_per_s": B * W * H / (ms * 1e-3), "fps": B * 1e3 / ms,
-           "samples_per_step": int(st.samples_emitted), "mlp_samples_per_s": st.samples_emitted / (ms_mlp * 1e-3),
-           "ms_mlp": ms_mlp, "chunks": int(st.chunks)}
-    if precision == "bf16":
-        out["mlp_frac_of_bf16_sustained"] = st.samples_emitted * fl / (ms_mlp * 1e-3) / 1e12 / peaks["bf16_sustained"]
-        # the sustained figure is cuBLAS under its own power throttle; a kernel that holds the full clock can pass it
-        out["mlp_frac_of_bf16_burst"] = st.samples_emitted * fl / (ms_mlp * 1e-3) / 1e12 / peaks["bf16"]
+        ms.append(e0.elapsed_time(e1))
+        for k in STAGES:
+            stage[k].append(getattr(st, k))
+    med = statistics.median(ms)
+    stage_med = {k: statistics.median(v) for k, v in stage.items()}
+    out = {"config": config, "name": sc.name + (" (pinhole view)" if pinhole else "") + (" (stereo pair)" if stereo else ""),
+           "image": [W, H], "poses": B, "n_subfields": sc.n_subfields,
+           "mlp": [sc.n_hidden, sc.hidden_width], "K": sc.samples_per_voxel, "precision": precision, "steps": steps,
+           "ms_per_step": med, "ms_per_step_mean": sum(ms) / len(ms), "rays_per_s": B * W * H / (med * 1e-3),
+           "fps": B * 1e3 / med, "samples_per_step": int(st.samples_emitted), "segments_per_step": int(st.segments),
+           "mlp_samples_per_s": st.samples_emitted / (stage_med["ms_mlp"] * 1e-3) if stage_med["ms_mlp"] > 0 else None,
+           "stage_ms": stage_med, "chunks": int(st.chunks), "kernel_launches": int(st.kernel_launches),
+           "roofline": mlp_roofline(sc, precision, st.samples_emitted, stage_med["ms_mlp"], peaks, alu_peak),
+           "hbm_stages": hbm_stage_table(sc, precision, W, H, B, int(st.segments), stage_med, peaks, False)}
     scene.close()
     del rgb, depth, flush
     torch.cuda.empty_cache()
@@ -251,15 +333,18 @@ def time_extras(r360, config):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
-    ap.add_argument("--precision", default="auto", choices=["auto", "fp32", "bf16"])
+    ap.add_argument("--precision", default="auto", choices=["auto", "fp32", "bf16", "f16"])
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"])
     ap.add_argument("--ref-row-stride", type=int, default=8)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="skip the short device-timed entries of configs 4, 5 and of this config's other precisions")
     ap.add_argument("--all-configs", action="store_true",
-                    help="also time BASELINE.json's other configs (short runs) and add them as other_configs")
+                    help="also time configs 1, 2, the 720p pinhole view, a stereo pair and the stand-alone entry points")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -278,25 +363,33 @@ def main():
     import paper_2208_02705_b200 as r360
     if not os.path.exists(r360.lib_path()):
         g.build()
+    from paper_2208_02705_b200.shard import rank_pose, render_sharded
     from scenegen import make_scene
     sc = make_scene(args.config)
     scene = r360.scene_from(sc)
     precision = args.precision
     if precision == "auto":
         try:
-            scene.set_precision("bf16")
+            scene.set_precision("bf16")          # BASELINE.json's "bf16 tensor-core variant"
             precision = "bf16"
         except r360.R360Error:
             precision = "fp32"
     scene.set_precision(precision)
     scene.use_current_torch_stream()
-    # each rank renders its own pose: rank r yaws pose 0 by r * 2pi/world about the world up axis
-    from paper_2208_02705_b200.shard import rank_pose
-    pose = rank_pose(sc.poses[0], rank, world)
+    strong = args.scaling == "strong"
+    # weak: each rank renders its own pose (rank r yaws pose 0 by r * 2pi/world about the world up axis);
+    # strong: every rank renders its band of the SAME frame
+    pose = np.asarray(sc.poses[0], np.float32) if strong else rank_pose(sc.poses[0], rank, world)
     W, H = sc.W, sc.H
     rgb = torch.empty((1, H, W, 3), dtype=torch.float32, device="cuda")
     depth = torch.empty((1, H, W), dtype=torch.float32, device="cuda")
     flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda")
+
+    def step():
+        if strong:
+            render_sharded(scene.render_rows, pose, W, H, rank, world, dist, rgb[0], depth[0])
+        else:
+            scene.render(pose, W, H, rgb, depth)      # r360_render + r360_wait (no wait for the frame itself)
 
     def barrier():
         if use_dist:
@@ -304,108 +397,131 @@ def main():
         torch.cuda.synchronize()
 
     for _ in range(args.warmup):
-        scene.render(pose, W, H, rgb, depth)
+        step()
     barrier()
     clocks = ClockSampler(local)
     clocks.start()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
-    stage = {k: 0.0 for k in ("ms_count", "ms_scan", "ms_emit", "ms_mlp", "ms_composite")}
+    stage = {k: [] for k in STAGES}
     launches = 0
     barrier()
     for k in range(args.steps):
         flush.zero_()
         ev[k][0].record()
-        scene.render(pose, W, H, rgb, depth)
+        step()
         ev[k][1].record()
         st = scene.stats()                      # synchronises; per-stage CUDA events on the launch stream
-        for key in stage:
-            stage[key] += getattr(st, key)
+        for key in STAGES:
+            stage[key].append(getattr(st, key))
         launches += st.kernel_launches
     barrier()
     clk = clocks.stop()
-    ms_total = sum(a.elapsed_time(b) for a, b in ev)
-    tt = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    tt = torch.tensor([sum(step_ms), statistics.median(step_ms)], dtype=torch.float64, device="cuda")
     if use_dist:
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-    ms_step = float(tt.item()) / args.steps
-    rays_step = W * H * world
+    ms_step = float(tt[0].item()) / args.steps
+    ms_median = float(tt[1].item())
+    rays_step = W * H * (1 if strong else world)
     value = rays_step / (ms_step * 1e-3)
 
     # end to end through the host-buffer entry point (pinned host buffers, H2D pose + D2H image per step)
-    h_rgb = torch.empty((1, H, W, 3), dtype=torch.float32).pin_memory()
-    h_depth = torch.empty((1, H, W), dtype=torch.float32).pin_memory()
-    h_pose = torch.from_numpy(pose.copy()).pin_memory()
-    for _ in range(2):
-        scene.render_batch_host(h_pose.numpy(), W, H, h_rgb.numpy(), h_depth.numpy())
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        scene.render_batch_host(h_pose.numpy(), W, H, h_rgb.numpy(), h_depth.numpy())
-    torch.cuda.synchronize()
-    te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-    if use_dist:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = rays_step * args.steps / float(te.item())
+    def e2e_loop(fmt, stream_frames=False):
+        scene.set_output_format(fmt)
+        t_rgb, t_d = (torch.float32, torch.float32) if fmt == "f32" else (torch.uint8, torch.float16)
+        h_rgb = torch.empty((1, H, W, 3), dtype=t_rgb).pin_memory()
+        h_depth = torch.empty((1, H, W), dtype=t_d).pin_memory()
+        h_rgb2 = torch.empty((1, H, W, 3), dtype=t_rgb).pin_memory() if stream_frames else None
+        h_depth2 = torch.empty((1, H, W), dtype=t_d).pin_memory() if stream_frames else None
+        n_done = [0]
+        h_pose = torch.from_numpy(np.ascontiguousarray(pose).copy()).pin_memory()
+        if strong:
+            d_rgb = torch.empty((H, W, 3), dtype=t_rgb, device="cuda")
+            d_d = torch.empty((H, W), dtype=t_d, device="cuda")
+
+        def one():
+            if strong:      # band + all-gather on the device, then the whole frame to the host
+                render_sharded(scene.render_rows, h_pose.numpy(), W, H, rank, world, dist, d_rgb, d_d)
+                h_rgb[0].copy_(d_rgb, non_blocking=True)
+                h_depth[0].copy_(d_d, non_blocking=True)
+                torch.cuda.synchronize()
+            elif stream_frames:   # a stream of frames: frame k's copy runs behind frame k+1's kernels
+                a, b = (h_rgb, h_depth) if n_done[0] % 2 == 0 else (h_rgb2, h_depth2)
+                n_done[0] += 1
+                scene.render_batch_host(h_pose.numpy(), W, H, a.numpy(), b.numpy(), sync=False)
+            else:
+                scene.render_batch_host(h_pose.numpy(), W, H, h_rgb.numpy(), h_depth.numpy())
+        for _ in range(3):
+            one()
+        if stream_frames:
+            scene.host_sync()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            one()
+        if stream_frames:
+            scene.host_sync()        # every frame of the timed region is in host memory
+        torch.cuda.synchronize()
+        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
+        if use_dist:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        scene.set_output_format("f32")
+        bytes_px = 16 if fmt == "f32" else 5
+        return {"value": rays_step * args.steps / float(te.item()), "unit": "rays/s",
+                "ms_per_step": 1e3 * float(te.item()) / args.steps,
+                "h2d_bytes_per_step": 48 * world, "d2h_bytes_per_step": W * H * bytes_px * world,
+                "output": "rgb float32 x 3 + depth float32" if fmt == "f32" else "rgb uint8 x 3 + depth binary16",
+                "call": "r360_render_rows + NCCL all-gather + copy to pinned host" if strong else
+                        ("r360_render_batch_host_async per frame + one r360_host_sync at the end (a stream of frames: "
+                         "each frame's copy runs behind the next frame's kernels)" if stream_frames else
+                         "r360_render_batch_host (synchronous: returns when the frame is in the pinned host buffers)")}
+    e2e = e2e_loop("f32")
+    e2e_small = e2e_loop("rgb8_d16")
+    e2e_stream = None if strong else e2e_loop("f32", stream_frames=True)
 
     if rank == 0:
         peaks = measured_peaks()
+        tf, mhz = r360.measure_fp32_fma()
+        alu_peak = {"tflops": tf, "source": f"measured on this GPU: r360_measure_fp32_fma (register-only FMA kernel, "
+                                            f"best of 5), nominal SM clock {mhz:.0f} MHz"}
         samples = st.samples_emitted
-        ms_mlp = stage["ms_mlp"] / args.steps
-        fl = flop_per_sample(sc.hidden_width, sc.n_hidden)
-        ach = samples * fl / (ms_mlp * 1e-3) / 1e12
-        if precision == "bf16":
-            roof = {"bound": "tensor", "kernel": "k_mlp_tc", "achieved": ach, "peak": peaks["bf16_sustained"],
-                    "unit": "TFLOP/s", "frac": ach / peaks["bf16_sustained"], "traffic": None,
-                    "peak_source": peaks["source"] + " bf16 sustained (kernel timed inside a long step)"}
-        else:
-            roof = {"bound": "alu", "kernel": "k_mlp_fp32", "achieved": ach, "peak": ALU_PEAK_TFLOPS,
-                    "unit": "TFLOP/s", "frac": ach / ALU_PEAK_TFLOPS, "traffic": None,
-                    "peak_source": "derived: 148 SM x 128 FMA/clk x 2 x 1.965 GHz"}
-        roof["flop_per_sample"] = fl
-        if precision == "bf16" and args.config == 3:
+        stage_med = {k: statistics.median(v) for k, v in stage.items()}
+        roof = mlp_roofline(sc, precision, samples, stage_med["ms_mlp"], peaks, alu_peak)
+        on_capture = precision == "bf16" and args.config == 3 and not strong     # what the committed ncu capture ran
+        if on_capture:
             roof["traffic"] = ncu_traffic("k_mlp_tc")
-        if precision == "bf16":
-            # MEASURED_PEAKS.json's sustained figure is a power-throttled cuBLAS run (its clocks_under_load block);
-            # the fraction of the burst figure is reported beside it
-            roof["peak_burst"] = peaks["bf16"]
-            roof["frac_of_burst"] = ach / peaks["bf16"]
-            roof["executed_flop_per_sample"] = executed_flop_per_sample(sc.hidden_width, sc.n_hidden)
-        roof["samples_per_launch"] = int(samples)
-        roof["ms_per_launch"] = ms_mlp
-        # the memory-side stages against the measured HBM copy bandwidth: algorithmic bytes
-        rays, segs, Kk = W * H, int(st.segments), sc.samples_per_voxel
-        tensor = precision == "bf16"
-        stage_bytes = {
-            "k_count": rays * 8 + segs * 10 + (rays * 64 if tensor else 0),
-            "k_emit": rays * 8 + segs * 10 + segs * (40 if tensor else 24),
-            "k_composite": segs * Kk * (8 if tensor else 16) + segs * 8 + rays * 24,   # tensor path: binary16 x4 per sample
-        }
-        stage_key = {"k_count": "ms_count", "k_emit": "ms_emit", "k_composite": "ms_composite"}
-        hbm_stages = {}
-        for kname, nbytes in stage_bytes.items():
-            ms_k = stage[stage_key[kname]] / args.steps
-            gbs = nbytes / (ms_k * 1e-3) / 1e9 if ms_k > 0 else 0.0
-            hbm_stages[kname] = {"algorithmic_bytes": int(nbytes), "ms": ms_k, "achieved_gbs": gbs,
-                                 "frac_of_hbm_peak": gbs / peaks["hbm"],
-                                 # the committed ncu captures are of config 3 on the tensor path only
-                                 "traffic": ncu_traffic(kname) if tensor and args.config == 3 else None}
         line = {"metric": "rays_per_second_equirect_render", "value": value, "unit": "rays/s", "n_gpus": world,
-                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": "bf16" if precision == "bf16" else "f32",
-                "data": "synthetic", "config": workload_config(sc, args, precision),
-                "fps": 1e3 / ms_step * world, "mlp_samples_per_s": samples / (ms_mlp * 1e-3),
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "ms_per_step_median": ms_median,
+                "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
+                "dtype": {"bf16": "bf16", "f16": "f16", "fp32": "f32"}[precision],
+                "data": "synthetic", "config": workload_config(sc, args), "precision": precision,
+                "fps": 1e3 / ms_step * (1 if strong else world),
+                "mlp_samples_per_s": samples / (stage_med["ms_mlp"] * 1e-3),
                 "samples_per_frame": int(samples), "segments_per_frame": int(st.segments),
-                "stage_ms": {k: v / args.steps for k, v in stage.items()},
-                "clocks": clk, "roofline": roof, "hbm_stages": hbm_stages,
-                "e2e": {"value": e2e_value, "unit": "rays/s", "h2d_bytes_per_step": 48 * world,
-                        "d2h_bytes_per_step": W * H * 16 * world},
-                "gpu_launches": int(launches)}
+                "stage_ms": stage_med, "stage_ms_note": "median over the timed steps of the per-stage CUDA events "
+                                                        "(r360_get_stats), rank 0",
+                "clocks": clk, "roofline": roof,
+                "hbm_stages": hbm_stage_table(sc, precision, W, H if not strong else -(-H // world), 1, int(st.segments),
+                                              stage_med, peaks, on_capture),
+                "e2e": e2e, "e2e_rgb8_d16": e2e_small, "e2e_stream_of_frames": e2e_stream,
+                "gpu_launches": int(launches), "retries": int(st.retries)}
+        scene.close()
+        del rgb, depth
+        torch.cuda.empty_cache()
+        if not args.no_other_configs:
+            # the other numbers DESIGN.md / BASELINE.md quote, measured by this same run (short, device-timed)
+            others = [time_config(r360, args.config, p, peaks, alu_peak, steps=3 if p == "fp32" else 10)
+                      for p in ("bf16", "f16", "fp32") if p != precision]
+            others += [time_config(r360, c, "bf16", peaks, alu_peak, steps=3 if c == 4 else 5) for c in (4, 5)
+                       if c != args.config]
+            line["other_configs"] = others
         if args.all_configs:
-            scene.close()
-            del rgb, depth
-            line["other_configs"] = [time_config(r360, c, precision) for c in (1, 2, 4, 5) if c != args.config]
+            more = [time_config(r360, c, precision, peaks, alu_peak) for c in (1, 2) if c != args.config]
             # the paper times its perspective (roaming) view at 720p: same scene, 90 degree pinhole
-            line["other_configs"].append(time_config(r360, args.config, precision, pinhole=(1280, 720, 640.0)))
+            more.append(time_config(r360, args.config, precision, peaks, alu_peak, pinhole=(1280, 720, 640.0)))
+            # stereoscopic mode: two eyes in one batch, against two mono frames
+            more.append(time_config(r360, args.config, precision, peaks, alu_peak, stereo=True))
+            line["more_configs"] = more
             line["extras"] = time_extras(r360, args.config)
         if not args.no_cpu_baseline:
             cb = oracle_sample(sc, args.ref_row_stride)
@@ -413,6 +529,7 @@ def main():
                                     "kind": "oracle", "sample": cb["sample"]}
         print(json.dumps(line), flush=True)
     if use_dist:
+        dist.barrier()
         dist.destroy_process_group()
 
 

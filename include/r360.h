@@ -121,11 +121,23 @@ r360_status r360_render_rows(r360_scene* scene, const float pose[12], int32_t W,
 
 /* End-to-end call: like r360_render_batch but the outputs are HOST buffers ([B*H*W*3], [B*H*W] in the
  * scene's output format; pinned memory for full PCIe speed).  Every chunk of rays (r360_set_chunk_rays; a call
- * that fits one chunk is cut into r360_set_host_bands bands, default 4) is copied device -> host on a second
+ * that fits one chunk can be cut into bands, r360_set_host_bands) is copied device -> host on a second
  * stream while the next chunk is rendered; the call returns when all copies are done, also after an error. */
 r360_status r360_render_batch_host(r360_scene* scene, const float* poses, int32_t B, int32_t W, int32_t H,
                                    void* out_rgb_host, void* out_depth_host);
-r360_status r360_set_host_bands(r360_scene* scene, int32_t bands /* 1..64 */);
+/* A call that fits one ray chunk can be cut into `bands` (1..64) chunks so that a band's copy runs behind the next
+ * band's kernels.  Default 1: measured on config 3 (2048 x 1024), every extra chunk costs 0.13 ms of kernel tails,
+ * more than the copy it hides. */
+r360_status r360_set_host_bands(r360_scene* scene, int32_t bands);
+
+/* Streaming form of r360_render_batch_host: returns when the frame and its copy to the host are enqueued.  Two
+ * staging buffers are used in turn, so the copy of one frame runs behind the kernels of the next: a stream of
+ * frames costs max(render, copy) per frame instead of their sum.  The host buffers of a call must stay valid, and
+ * hold the frame, once r360_host_sync (or the second-next r360_render_batch_host_async) has returned. */
+r360_status r360_render_batch_host_async(r360_scene* scene, const float* poses, int32_t B, int32_t W, int32_t H,
+                                         void* out_rgb_host, void* out_depth_host);
+/* Waits until every frame enqueued by r360_render_batch_host_async is in its host buffers. */
+r360_status r360_host_sync(r360_scene* scene);
 
 /* Returns once the outputs of the last render call are guaranteed complete IN STREAM ORDER (see "Conventions"):
  * waits for the frame's sample count, re-renders a chunk whose samples exceeded the buffers.  Does not wait for
@@ -255,6 +267,11 @@ r360_status r360_get_stats(r360_scene* scene, r360_stats* out);
 r360_status r360_debug_samples(r360_scene* scene, const float pose[12], int32_t W, int32_t H,
                                uint32_t* counts, uint32_t* offsets, float* t, int32_t* subfield,
                                uint64_t cap, uint64_t* total);
+
+/* Measurement helper for bench.py: the FP32 FMA rate of the current device in TFLOP/s (2 FLOP per FMA; best of five
+ * launches of a register-only FMA kernel that fills every SM), the roofline of the fp32 MLP path.
+ * sm_mhz_out (may be NULL) receives the device's nominal SM clock. */
+r360_status r360_measure_fp32_fma(double* tflops_out, double* sm_mhz_out);
 
 const char* r360_status_string(r360_status s);
 /* Text of the last CUDA error seen by this library on the calling thread ("" if none). */

@@ -6,8 +6,8 @@ sm_100a).  Argument marshalling only: every step of the path runs in the CUDA ke
 There is no CPU fallback; loading fails loudly if the library is missing.
 """
 from .binding import (R360Error, Scene, Stats, assign_subfields, floorplan, occupancy_fuse, lib,
-                      lib_path, params_per_subfield, scene_from,
+                      lib_path, measure_fp32_fma, params_per_subfield, scene_from,
                       version, STATUS)
 
-__all__ = ["R360Error", "Scene", "Stats", "assign_subfields", "floorplan", "occupancy_fuse", "lib", "lib_path", "params_per_subfield", "scene_from", "version",
+__all__ = ["R360Error", "Scene", "Stats", "assign_subfields", "floorplan", "occupancy_fuse", "lib", "lib_path", "measure_fp32_fma", "params_per_subfield", "scene_from", "version",
            "STATUS"]

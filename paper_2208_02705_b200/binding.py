@@ -65,6 +65,10 @@ def lib():
     L.r360_render_batch.argtypes = [vp, f32p, i32, i32, i32, vp, vp]
     L.r360_render_batch_host.restype = C.c_int
     L.r360_render_batch_host.argtypes = [vp, f32p, i32, i32, i32, vp, vp]
+    L.r360_render_batch_host_async.restype = C.c_int
+    L.r360_render_batch_host_async.argtypes = [vp, f32p, i32, i32, i32, vp, vp]
+    L.r360_host_sync.restype = C.c_int
+    L.r360_host_sync.argtypes = [vp]
     L.r360_render_rows.restype = C.c_int
     L.r360_render_rows.argtypes = [vp, f32p, i32, i32, i32, i32, vp, vp]
     for name in ("r360_wait", "r360_graph_status"):
@@ -77,6 +81,8 @@ def lib():
     L.r360_reserve.argtypes = [vp, C.c_uint64, C.c_double]
     L.r360_set_graph_poses.restype = C.c_int
     L.r360_set_graph_poses.argtypes = [vp, f32p, i32]
+    L.r360_measure_fp32_fma.restype = C.c_int
+    L.r360_measure_fp32_fma.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.r360_set_precision.restype = C.c_int
     L.r360_set_precision.argtypes = [vp, i32]
     L.r360_assign_subfields.restype = C.c_int
@@ -109,6 +115,13 @@ def lib():
 
 def version():
     return lib().r360_version().decode()
+
+
+def measure_fp32_fma():
+    """(TFLOP/s, nominal SM MHz) of the FP32 FMA pipes of the current device (r360_measure_fp32_fma)."""
+    tf, mhz = C.c_double(0), C.c_double(0)
+    _check(lib().r360_measure_fp32_fma(C.byref(tf), C.byref(mhz)), "r360_measure_fp32_fma")
+    return tf.value, mhz.value
 
 
 def _check(st, where):
@@ -308,8 +321,12 @@ class Scene:
             self.wait()
         return out_rgb, out_depth
 
-    def render_batch_host(self, poses, W, H, out_rgb=None, out_depth=None):
-        """HOST buffers in and out (numpy, ideally pinned): the end-to-end call."""
+    def host_sync(self):
+        _check(lib().r360_host_sync(self._h), "r360_host_sync")
+
+    def render_batch_host(self, poses, W, H, out_rgb=None, out_depth=None, sync=True):
+        """HOST buffers in and out (numpy, ideally pinned): the end-to-end call.  sync=False: the streaming form
+        (r360_render_batch_host_async); the buffers hold the frame after host_sync()."""
         poses = np.asarray(poses, np.float32)
         B = poses.size // 12
         fmt = getattr(self, "_fmt", 0)
@@ -321,8 +338,8 @@ class Scene:
         assert out_rgb.dtype == t_rgb and out_depth.dtype == t_d
         assert out_rgb.size == B * H * W * 3 and out_depth.size == B * H * W
         keep, p = _pose_ptr(poses, B)
-        st = lib().r360_render_batch_host(self._h, p, B, W, H, out_rgb.ctypes.data, out_depth.ctypes.data)
-        _check(st, "r360_render_batch_host")
+        fn = lib().r360_render_batch_host if sync else lib().r360_render_batch_host_async
+        _check(fn(self._h, p, B, W, H, out_rgb.ctypes.data, out_depth.ctypes.data), "r360_render_batch_host")
         return out_rgb, out_depth
 
     def stats(self):

@@ -6,7 +6,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(CSRC, "libr360.so")
-SOURCES = ["capi.cu", "render.cu", "sampler.cu", "mlp_fp32.cu", "mlp_tc.cu", "composite.cu", "assign.cu", "floorplan.cu", "fuse.cu"]
+SOURCES = ["capi.cu", "render.cu", "sampler.cu", "mlp_fp32.cu", "mlp_tc.cu", "composite.cu", "assign.cu", "floorplan.cu", "fuse.cu", "microbench.cu"]
 HEADERS = sorted(f for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))) + [os.path.join("..", "..", "include", "r360.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-fno-fast-math,-Wall", "--shared", "-cudart", "static"]

@@ -164,7 +164,10 @@ void r360_scene_destroy(r360_scene* sc) {
   cudaFree(sc->buf.hit_t); cudaFree(sc->buf.hit_lab);
   cudaFree(sc->buf.bin_ovf); cudaFree(sc->buf.blk_list); cudaFree(sc->buf.blk_list_n);
   cudaFree(sc->d_pass_cnt); cudaFree(sc->buf.pass_off); cudaFree(sc->buf.st_c); cudaFree(sc->buf.st_T);
-  cudaFree(sc->d_stage_rgb); cudaFree(sc->d_stage_depth);
+  for (int i = 0; i < 2; ++i) {
+    cudaFree(sc->d_stage_rgb[i]); cudaFree(sc->d_stage_depth[i]);
+    if (sc->ev_copy_done[i]) cudaEventDestroy(sc->ev_copy_done[i]);
+  }
   if (sc->h_snap) cudaFreeHost(sc->h_snap);
   if (sc->h_poses) cudaFreeHost(sc->h_poses);
   if (sc->copy_stream) cudaStreamDestroy(sc->copy_stream);

@@ -169,24 +169,18 @@ __device__ __forceinline__ void pe_recurrence(const float x[3], float* out) {
 // rows of the hidden layers (first 16 entries = one K step), the whole block feeds the colour layer.
 constexpr int kDirBlockWords = 16;
 
-__device__ __forceinline__ void store_dir_block(uint4* dst, const float d[3], bool f16) {
+template <bool F16>
+__device__ __forceinline__ void store_dir_block(uint4* dst, const float d[3]) {
   float pd[32];
   pd[0] = 1.0f;
   pd[1] = 1.0f;
   pe_recurrence<kTcLd>(d, pd + 2);
 #pragma unroll
   for (int c = 2 + kTcPeD; c < 32; ++c) pd[c] = 0.0f;
-  if (f16) {
 #pragma unroll
-    for (int c = 0; c < 4; ++c)
-      dst[c] = make_uint4(pack_f16(pd[8 * c], pd[8 * c + 1]), pack_f16(pd[8 * c + 2], pd[8 * c + 3]),
-                          pack_f16(pd[8 * c + 4], pd[8 * c + 5]), pack_f16(pd[8 * c + 6], pd[8 * c + 7]));
-  } else {
-#pragma unroll
-    for (int c = 0; c < 4; ++c)
-      dst[c] = make_uint4(pack_bf16(pd[8 * c], pd[8 * c + 1]), pack_bf16(pd[8 * c + 2], pd[8 * c + 3]),
-                          pack_bf16(pd[8 * c + 4], pd[8 * c + 5]), pack_bf16(pd[8 * c + 6], pd[8 * c + 7]));
-  }
+  for (int c = 0; c < 4; ++c)
+    dst[c] = make_uint4(pack16<F16>(pd[8 * c], pd[8 * c + 1]), pack16<F16>(pd[8 * c + 2], pd[8 * c + 3]),
+                        pack16<F16>(pd[8 * c + 4], pd[8 * c + 5]), pack16<F16>(pd[8 * c + 6], pd[8 * c + 7]));
 }
 
 }  // namespace r360

@@ -326,7 +326,10 @@ r360_status r360_settle(r360_scene* sc, bool block) {
       sc->stats.kernel_launches += launches;
       sc->retries += 1;
       if (st != R360_OK) { pd.chunks.clear(); pd.next = 0; return st; }
-      if (pd.host_rgb) enqueue_host_copy(sc, pd, job);
+      if (pd.host_rgb) {
+        enqueue_host_copy(sc, pd, job);
+        if (pd.copy_done) cudaEventRecord(pd.copy_done, sc->copy_stream);
+      }
     }
   }
   return R360_OK;
@@ -360,6 +363,7 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
   pd.next = 0;
   pd.W = W; pd.H = H;
   pd.out_rgb = out_rgb; pd.out_depth = out_depth; pd.host_rgb = host_rgb; pd.host_depth = host_depth;
+  if (!host_rgb) pd.copy_done = nullptr;
   pd.out_format = sc->out_format;
   r360_stats& stats = sc->stats;
   std::memset(&stats, 0, sizeof(stats));
@@ -405,36 +409,57 @@ r360_status r360_render_rows(r360_scene* sc, const float pose[12], int32_t W, in
   return render_device(sc, pose, 1, W, H, (long long)row0 * W, (long long)row1 * W, out_rgb, out_depth);
 }
 
-r360_status r360_render_batch_host(r360_scene* sc, const float* poses, int32_t B, int32_t W, int32_t H,
-                                   void* out_rgb_host, void* out_depth_host) {
+r360_status r360_render_batch_host_async(r360_scene* sc, const float* poses, int32_t B, int32_t W, int32_t H,
+                                         void* out_rgb_host, void* out_depth_host) {
   if (!sc || !poses || !out_rgb_host || !out_depth_host || B < 1 || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
   if (capturing(sc->stream)) return R360_ERR_INVALID_ARG;
   r360_status st;
-  if ((st = r360_settle(sc, true)) != R360_OK) return st;
-  const size_t R = (size_t)B * W * H;
-  if (R > sc->stage_rays_cap) {
-    cudaFree(sc->d_stage_rgb); cudaFree(sc->d_stage_depth);
-    sc->d_stage_rgb = sc->d_stage_depth = nullptr;
-    sc->stage_rays_cap = 0;
-    R360_CUDA(cudaMalloc(&sc->d_stage_rgb, R * 3 * sizeof(float)));
-    R360_CUDA(cudaMalloc(&sc->d_stage_depth, R * sizeof(float)));
-    sc->stage_rays_cap = R;
-  }
+  if ((st = r360_settle(sc, true)) != R360_OK) return st;       // (re-renders and re-copies the previous frame if needed)
   if (!sc->copy_stream) {
     R360_CUDA(cudaStreamCreateWithFlags(&sc->copy_stream, cudaStreamNonBlocking));
     R360_CUDA(cudaEventCreateWithFlags(&sc->ev_chunk_done, cudaEventDisableTiming));
+    for (auto& e : sc->ev_copy_done) R360_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
   }
-  st = render_device(sc, poses, B, W, H, 0, (long long)R, sc->d_stage_rgb, sc->d_stage_depth, out_rgb_host,
+  const int cur = sc->stage_idx ^= 1;
+  const size_t R = (size_t)B * W * H;
+  if (R > sc->stage_rays_cap[cur]) {
+    cudaFree(sc->d_stage_rgb[cur]); cudaFree(sc->d_stage_depth[cur]);
+    sc->d_stage_rgb[cur] = sc->d_stage_depth[cur] = nullptr;
+    sc->stage_rays_cap[cur] = 0;
+    R360_CUDA(cudaMalloc(&sc->d_stage_rgb[cur], R * 3 * sizeof(float)));
+    R360_CUDA(cudaMalloc(&sc->d_stage_depth[cur], R * sizeof(float)));
+    sc->stage_rays_cap[cur] = R;
+  }
+  // this staging set was last used two frames ago: its copy must have left before the kernels overwrite it
+  R360_CUDA(cudaStreamWaitEvent(sc->stream, sc->ev_copy_done[cur], 0));
+  sc->pending.copy_done = sc->ev_copy_done[cur];
+  st = render_device(sc, poses, B, W, H, 0, (long long)R, sc->d_stage_rgb[cur], sc->d_stage_depth[cur], out_rgb_host,
                      out_depth_host, sc->host_bands);
+  cudaEventRecord(sc->ev_copy_done[cur], sc->copy_stream);
+  return st;
+}
+
+r360_status r360_host_sync(r360_scene* sc) {
+  if (!sc) return R360_ERR_INVALID_ARG;
   // a chunk that overflowed is rendered and copied again here
-  if (st == R360_OK) st = r360_settle(sc, true);
+  r360_status st = r360_settle(sc, true);
   // on an error too: no copy may still be writing the caller's buffers when this returns
-  cudaError_t e2 = cudaStreamSynchronize(sc->stream), e1 = cudaStreamSynchronize(sc->copy_stream);
+  cudaError_t e2 = cudaStreamSynchronize(sc->stream);
+  cudaError_t e1 = sc->copy_stream ? cudaStreamSynchronize(sc->copy_stream) : cudaSuccess;
   sc->pending.host_rgb = sc->pending.host_depth = nullptr;
+  sc->pending.copy_done = nullptr;
   if (st != R360_OK) return st;
   if (e1 != cudaSuccess) return r360_cuda_fail(e1, "cudaStreamSynchronize(copy_stream)");
   if (e2 != cudaSuccess) return r360_cuda_fail(e2, "cudaStreamSynchronize(stream)");
   return R360_OK;
+}
+
+r360_status r360_render_batch_host(r360_scene* sc, const float* poses, int32_t B, int32_t W, int32_t H,
+                                   void* out_rgb_host, void* out_depth_host) {
+  r360_status st = r360_render_batch_host_async(sc, poses, B, W, H, out_rgb_host, out_depth_host);
+  if (st == R360_ERR_INVALID_ARG && (!sc || !poses || !out_rgb_host || !out_depth_host || B < 1 || W < 1 || H < 1)) return st;
+  r360_status st2 = sc ? r360_host_sync(sc) : R360_ERR_INVALID_ARG;
+  return st != R360_OK ? st : st2;
 }
 
 r360_status r360_wait(r360_scene* sc) {

@@ -84,6 +84,9 @@ __device__ __forceinline__ void reserve_bins(const ChunkBuffers& b, const uint32
 }
 
 // ---------------------------------------------------------------------------------------
+// DIR: 0 = no direction blocks (fp32 path), 1 = bfloat16, 2 = binary16 (a template parameter: with a run-time
+// format the two conversion paths cost the walk six registers and a resident block per SM)
+template <int DIR>
 __global__ void __launch_bounds__(kSamplerThreads)
 k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuffers b, int n_bins,
         int use_smem_hist) {
@@ -100,7 +103,7 @@ k_count(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuf
   if (valid) {
     const Ray ray = make_ray(f, r);
     w.init(g, ray);
-    if (b.dirblk) store_dir_block(b.dirblk + (size_t)r * 4, ray.d, b.dir_f16 != 0);   // tensor path: F(d) once per ray
+    if constexpr (DIR != 0) store_dir_block<DIR == 2>(b.dirblk + (size_t)r * 4, ray.d);   // tensor path: F(d) once per ray
   }
   uint32_t cnt = 0;
   // lock-step over "next occupied voxel" so the histogram update can be warp-aggregated
@@ -422,7 +425,9 @@ void launch_count(const GridParams& g, const uint16_t* grid, const FrameParams& 
   int blocks = (f.n_rays + kSamplerThreads - 1) / kSamplerThreads;
   int use_smem = n_bins <= 8192;
   size_t smem = use_smem ? (size_t)n_bins * sizeof(uint32_t) : 0;
-  k_count<<<blocks, kSamplerThreads, smem, s>>>(g, grid, f, b, n_bins, use_smem);
+  if (!b.dirblk) k_count<0><<<blocks, kSamplerThreads, smem, s>>>(g, grid, f, b, n_bins, use_smem);
+  else if (!b.dir_f16) k_count<1><<<blocks, kSamplerThreads, smem, s>>>(g, grid, f, b, n_bins, use_smem);
+  else k_count<2><<<blocks, kSamplerThreads, smem, s>>>(g, grid, f, b, n_bins, use_smem);
 }
 
 void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_tile, unsigned long long seg_cap,

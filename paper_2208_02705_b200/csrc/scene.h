@@ -44,16 +44,19 @@ struct r360_scene {
   double segs_per_ray_max = 0.0;            // largest segments-per-ray ratio of any chunk pass so far: sizes the buffers
   unsigned retries = 0;                     // chunks rendered again because their segments exceeded the capacity
   // D2H staging for r360_render_batch_host
-  float* d_stage_rgb = nullptr;
-  float* d_stage_depth = nullptr;
-  size_t stage_rays_cap = 0;
+  // two sets, used in turn: the copy of frame k runs behind the kernels of frame k+1 (r360_render_batch_host_async)
+  float* d_stage_rgb[2] = {nullptr, nullptr};
+  float* d_stage_depth[2] = {nullptr, nullptr};
+  size_t stage_rays_cap[2] = {0, 0};
+  cudaEvent_t ev_copy_done[2] = {nullptr, nullptr};   // recorded on copy_stream behind a frame's last copy
+  int stage_idx = 0;
   cudaStream_t copy_stream = nullptr;       // chunk k's image part goes to the host behind chunk k+1's kernels
   cudaEvent_t ev_chunk_done = nullptr;
   // configuration
   cudaStream_t stream = nullptr;
   int precision = 0;                        // 0 fp32 ALUs, 1 tensor cores bfloat16, 2 tensor cores binary16
   int out_format = 0;                       // r360_output_format
-  int host_bands = 4;                       // r360_render_batch_host cuts a single-chunk call into this many bands
+  int host_bands = 1;                       // r360_render_batch_host cuts a single-chunk call into this many bands
   int wavefront = 0;                        // r360_set_wavefront: feed the MLP in passes, retire finished rays between them
   uint32_t* d_pass_cnt = nullptr;           // owned; buf.pass_cnt points here only during wavefront passes
   size_t pass_cnt_cap = 0, pass_off_cap = 0, st_c_cap = 0, st_T_cap = 0;
@@ -69,6 +72,7 @@ struct r360_scene {
     unsigned next = 0;                      // first chunk not yet verified
     int W = 0, H = 0, out_format = 0;
     void *out_rgb = nullptr, *out_depth = nullptr, *host_rgb = nullptr, *host_depth = nullptr;
+    cudaEvent_t copy_done = nullptr;        // host output: re-recorded behind the copy of a re-rendered chunk
   } pending;
   r360_stats stats{};
 };

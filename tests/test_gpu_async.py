@@ -153,6 +153,37 @@ def test_host_bands_equal_single_copy(r360, scene2, bands):
     gpu.close()
 
 
+def test_streaming_host_output(r360, scene2):
+    """r360_render_batch_host_async: frames of a roaming path enqueued back to back, each copied to its own host
+    buffer behind the next frame's kernels; after r360_host_sync every buffer holds exactly the frame of the
+    synchronous call.  The third frame outgrows the buffers learnt from the first two (re-rendered, re-copied)."""
+    import torch
+    sc = scene2
+    gpu = r360.scene_from(sc)
+    gpu.set_precision("bf16")
+    poses = [_far_pose(sc), _far_pose(sc)]
+    for k in range(4):
+        p = sc.poses[0].copy()
+        p[3] += 0.15 * k
+        poses.append(p)
+    refs = []
+    ref_scene = r360.scene_from(sc)
+    ref_scene.set_precision("bf16")
+    for p in poses:
+        rgb, depth = ref_scene.render(p, sc.W, sc.H)
+        refs.append((rgb.cpu().numpy(), depth.cpu().numpy()))
+    bufs = [(torch.empty((1, sc.H, sc.W, 3), dtype=torch.float32).pin_memory(),
+             torch.empty((1, sc.H, sc.W), dtype=torch.float32).pin_memory()) for _ in poses]
+    for p, (h_rgb, h_d) in zip(poses, bufs):
+        gpu.render_batch_host(p, sc.W, sc.H, h_rgb.numpy(), h_d.numpy(), sync=False)
+    gpu.host_sync()
+    assert gpu.stats().retries >= 1
+    for (h_rgb, h_d), (rgb, depth) in zip(bufs, refs):
+        assert np.array_equal(h_rgb.numpy()[0], rgb) and np.array_equal(h_d.numpy()[0], depth)
+    gpu.close()
+    ref_scene.close()
+
+
 @pytest.mark.parametrize("precision", ["fp32", "bf16"])
 def test_stereo_pair_in_one_batch(r360, scene2, precision):
     """Stereoscopic mode: two eyes 65 mm apart along the camera's x axis, binned in ONE chunk
