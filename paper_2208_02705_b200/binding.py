@@ -236,8 +236,9 @@ class Scene:
         """"fp32" (FP32 ALUs), "bf16" (tensor cores, bfloat16 operands) or "f16" (tensor cores, binary16 operands)."""
         _check(lib().r360_set_precision(self._h, {"fp32": 0, "bf16": 1, "f16": 2}.get(mode, mode)), "r360_set_precision")
 
-    def set_wavefront(self, enable):
-        _check(lib().r360_set_wavefront(self._h, int(bool(enable))), "r360_set_wavefront")
+    def set_wavefront(self, mode):
+        """False / 0 = single pass, True / 1 = wavefronted passes, "auto" / 2 = passes iff the last frame was opaque."""
+        _check(lib().r360_set_wavefront(self._h, 2 if mode == "auto" else int(mode)), "r360_set_wavefront")
 
     def set_camera(self, model="equirect", fx=0.0, fy=0.0, cx=0.0, cy=0.0):
         _check(lib().r360_set_camera(self._h, {"equirect": 0, "pinhole": 1}.get(model, model), fx, fy, cx, cy),

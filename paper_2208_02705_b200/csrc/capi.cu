@@ -175,6 +175,7 @@ void r360_scene_destroy(r360_scene* sc) {
   for (auto& ce : sc->events) {
     for (auto& e : ce.e) cudaEventDestroy(e);
     cudaEventDestroy(ce.scanned);
+    cudaEventDestroy(ce.finished);
   }
   cudaGetLastError();
   delete sc;

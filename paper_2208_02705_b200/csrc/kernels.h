@@ -85,7 +85,10 @@ __device__ __forceinline__ bool chunk_cancelled(const ChunkBuffers& b) {
   return (b.totals[kTotOverflow] | b.totals[kTotWaveDone]) != 0;
 }
 
-constexpr int kSamplerThreads = 256;
+#ifndef R360_SAMPLER_THREADS
+#define R360_SAMPLER_THREADS 256
+#endif
+constexpr int kSamplerThreads = R360_SAMPLER_THREADS;   // rays per sampler block (k_count, k_emit, k_pass_count)
 
 // Wavefronted early termination: the hits of a ray are fed to the MLP in passes
 // [h0, h1) = [0,2) [2,6) [6,16) [16,kHitCap) [kHitCap, inf); after every pass the compositing kernel retires

@@ -132,6 +132,7 @@ r360_scene::ChunkEvents* chunk_events(r360_scene* sc, unsigned idx) {
     for (auto& e : ce.e)
       if (cudaEventCreate(&e) != cudaSuccess) return nullptr;
     if (cudaEventCreateWithFlags(&ce.scanned, cudaEventDisableTiming) != cudaSuccess) return nullptr;
+    if (cudaEventCreateWithFlags(&ce.finished, cudaEventDisableTiming) != cudaSuccess) return nullptr;
     try { sc->events.push_back(ce); } catch (const std::bad_alloc&) { return nullptr; }
   }
   return &sc->events[idx];
@@ -201,7 +202,7 @@ r360_status run_chunk(r360_scene* sc, int W, int H, const ChunkJob& job, unsigne
   if ((st = grow(sc->buf.blk_list, sc->blk_list_cap, n_blocks * kBlkListCap)) != R360_OK) return st;
   if ((st = grow(sc->buf.blk_list_n, sc->blk_list_n_cap, n_blocks)) != R360_OK) return st;
   sc->buf.pass_cnt = nullptr;
-  const bool wave = sc->wavefront && !sample_only;
+  const bool wave = sc->wave_now && !sample_only;
   if (wave) {
     if ((st = grow(sc->d_pass_cnt, sc->pass_cnt_cap, f.n_rays)) != R360_OK) return st;
     if ((st = grow(sc->buf.pass_off, sc->pass_off_cap, f.n_rays)) != R360_OK) return st;
@@ -286,6 +287,7 @@ r360_status run_chunk(r360_scene* sc, int W, int H, const ChunkJob& job, unsigne
   }
   // the chunk's counters for r360_get_stats
   R360_CUDA(cudaMemcpyAsync(snap_tot, sc->buf.totals, kTotN * sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
+  if (!cap) R360_CUDA(cudaEventRecord(ev->finished, s));
   return R360_OK;
 }
 
@@ -365,6 +367,15 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
   pd.out_rgb = out_rgb; pd.out_depth = out_depth; pd.host_rgb = host_rgb; pd.host_depth = host_depth;
   if (!host_rgb) pd.copy_done = nullptr;
   pd.out_format = sc->out_format;
+  // wavefront mode 2 (automatic): passes only if the last finished frame used less than half of its samples
+  // (opaque surfaces); a translucent scene, where every sample is needed, keeps the cheaper single pass
+  if (!cap && sc->chunks_last && sc->events.size() && cudaEventQuery(sc->events[0].finished) == cudaSuccess) {
+    const unsigned long long* snap = sc->h_snap + kTotN;        // chunk 0 of the last call
+    const unsigned long long emitted = (sc->wave_now ? snap[kTotGeo] : snap[kTotSegSum]) * (unsigned long long)sc->grid_p.K;
+    if (emitted) sc->used_ratio = (double)snap[kTotUsed] / (double)emitted;
+  }
+  cudaGetLastError();
+  if (!cap) sc->wave_now = sc->wavefront == 1 || (sc->wavefront == 2 && sc->used_ratio < 0.5);
   r360_stats& stats = sc->stats;
   std::memset(&stats, 0, sizeof(stats));
   stats.rays = (uint64_t)total_rays;
@@ -518,11 +529,13 @@ r360_status r360_set_host_bands(r360_scene* sc, int32_t bands) {
   return R360_OK;
 }
 
-r360_status r360_set_wavefront(r360_scene* sc, int32_t enable) {
-  if (!sc || (enable != 0 && enable != 1)) return R360_ERR_INVALID_ARG;
+r360_status r360_set_wavefront(r360_scene* sc, int32_t mode) {
+  if (!sc || mode < 0 || mode > 2) return R360_ERR_INVALID_ARG;
   r360_status st;
   if ((st = r360_settle(sc, true)) != R360_OK) return st;
-  sc->wavefront = enable;
+  sc->wavefront = mode;
+  sc->wave_now = mode == 1;
+  sc->used_ratio = 1.0;
   return R360_OK;
 }
 
@@ -574,7 +587,7 @@ r360_status r360_get_stats(r360_scene* sc, r360_stats* out) {
     st.mlp_tiles += snap[kTotTileSum];
     st.samples_used += snap[kTotUsed];
     // wavefront: `segments` counts what reached the MLP; the geometric total comes from the walk
-    st.samples_emitted += (sc->wavefront ? snap[kTotGeo] : snap[kTotSegSum]) * (uint64_t)sc->grid_p.K;
+    st.samples_emitted += (sc->wave_now ? snap[kTotGeo] : snap[kTotSegSum]) * (uint64_t)sc->grid_p.K;
   }
   cudaGetLastError();
   st.ms_total = st.ms_count + st.ms_scan + st.ms_emit + st.ms_mlp + st.ms_composite;

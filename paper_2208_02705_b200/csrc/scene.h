@@ -57,12 +57,14 @@ struct r360_scene {
   int precision = 0;                        // 0 fp32 ALUs, 1 tensor cores bfloat16, 2 tensor cores binary16
   int out_format = 0;                       // r360_output_format
   int host_bands = 1;                       // r360_render_batch_host cuts a single-chunk call into this many bands
+  bool wave_now = false;                    // what the current / last render call does
+  double used_ratio = 1.0;                  // samples composited / samples emitted of the last finished frame
   int wavefront = 0;                        // r360_set_wavefront: feed the MLP in passes, retire finished rays between them
   uint32_t* d_pass_cnt = nullptr;           // owned; buf.pass_cnt points here only during wavefront passes
   size_t pass_cnt_cap = 0, pass_off_cap = 0, st_c_cap = 0, st_T_cap = 0;
   long long chunk_rays = 4ll << 20;
   // statistics of the last call
-  struct ChunkEvents { cudaEvent_t e[6]; cudaEvent_t scanned; };
+  struct ChunkEvents { cudaEvent_t e[6]; cudaEvent_t scanned; cudaEvent_t finished; };
   std::vector<ChunkEvents> events;   // pool, one set per chunk
   unsigned chunks_last = 0;
   // the chunks enqueued by the last render call, until r360_settle has seen their overflow flags

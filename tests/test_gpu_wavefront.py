@@ -92,3 +92,24 @@ def test_wavefront_against_oracle(r360, oracle):
     check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 1e-4)
     assert gpu.stats().samples_emitted == int(ref["n_emitted"].sum())
     gpu.close()
+
+
+def test_automatic_mode_follows_the_scene(r360):
+    """r360_set_wavefront(2): passes only once a finished frame has shown that most samples go unused."""
+    import torch
+    sc = get_scene(5)
+    W, H = 512, 256
+    for bias, expect_passes in ((None, False), (40.0, True)):
+        gpu = r360.scene_from(sc) if bias is None else r360.scene_from(sc, weights=with_density_bias(sc, bias))
+        gpu.set_precision("bf16")
+        rgb0, d0 = gpu.render(sc.poses[0], W, H)
+        rgb0, d0 = rgb0.clone(), d0.clone()
+        gpu.set_wavefront("auto")
+        launches = []
+        for _ in range(3):
+            rgb, depth = gpu.render(sc.poses[0], W, H)
+            launches.append(gpu.stats().kernel_launches)            # synchronises: the next call sees this frame's ratio
+            assert torch.equal(rgb, rgb0) and torch.equal(depth, d0)
+        assert launches[0] == 5                                     # nothing known yet: single pass
+        assert (launches[-1] > 5) == expect_passes
+        gpu.close()
