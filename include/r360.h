@@ -202,6 +202,22 @@ r360_status r360_occupancy_fuse(const int32_t dims[3], const float box_min[3], c
                                 float* logodds, const float pose[12], int32_t W, int32_t H,
                                 const float* depth, const float* uncertainty);
 
+/* The same with the log-odds grid RESIDENT ON THE DEVICE between observations (Algorithm 1 stage I fuses the
+ * panoramas progressively): create once (logodds_init: HOST float[N] or NULL for zeros), fuse any
+ * number of observations (r360_fusion_fuse: HOST depth / uncertainty images; r360_fusion_fuse_device: DEVICE images,
+ * e.g. the depth output of r360_render), read back when needed (logodds_out: HOST float[N] or NULL; occupancy_out:
+ * HOST uint8[N] or NULL, 255 where logit > ln(0.97/0.03), else 0 -- the occupancy input of r360_scene_create with
+ * occ_threshold 128).  Work runs on the default stream of the current device; r360_fusion_read synchronises. */
+typedef struct r360_fusion r360_fusion;
+r360_status r360_fusion_create(const int32_t dims[3], const float box_min[3], const float box_max[3],
+                               const float* logodds_init, r360_fusion** out);
+r360_status r360_fusion_fuse(r360_fusion* fusion, const float pose[12], int32_t W, int32_t H, const float* depth,
+                             const float* uncertainty);
+r360_status r360_fusion_fuse_device(r360_fusion* fusion, const float pose[12], int32_t W, int32_t H,
+                                    const float* depth, const float* uncertainty);
+r360_status r360_fusion_read(r360_fusion* fusion, float* logodds_out, uint8_t* occupancy_out);
+void r360_fusion_destroy(r360_fusion* fusion);
+
 /* Camera of the following render / debug calls.  model 0 (default) = the equirectangular panorama of
  * Eq.2-3; model 1 = pinhole view for roaming (the paper's perspective display,
  * PAPER.md:206, :200, gives no model; reading P): pixel centre (i+0.5, j+0.5) ->

@@ -90,6 +90,16 @@ def lib():
                                         C.POINTER(C.c_int32)]
     L.r360_occupancy_fuse.restype = C.c_int
     L.r360_occupancy_fuse.argtypes = [C.POINTER(C.c_int32), f32p, f32p, f32p, f32p, i32, i32, f32p, f32p]
+    L.r360_fusion_create.restype = C.c_int
+    L.r360_fusion_create.argtypes = [C.POINTER(C.c_int32), f32p, f32p, f32p, C.POINTER(vp)]
+    L.r360_fusion_fuse.restype = C.c_int
+    L.r360_fusion_fuse.argtypes = [vp, f32p, i32, i32, f32p, f32p]
+    L.r360_fusion_fuse_device.restype = C.c_int
+    L.r360_fusion_fuse_device.argtypes = [vp, f32p, i32, i32, vp, vp]
+    L.r360_fusion_read.restype = C.c_int
+    L.r360_fusion_read.argtypes = [vp, f32p, C.POINTER(C.c_uint8)]
+    L.r360_fusion_destroy.restype = None
+    L.r360_fusion_destroy.argtypes = [vp]
     L.r360_floorplan.restype = C.c_int
     L.r360_floorplan.argtypes = [C.POINTER(C.c_int32), C.POINTER(C.c_uint8), C.c_uint8, i32, i32, f32p, f32p,
                                  C.POINTER(C.c_uint8)]
@@ -176,6 +186,57 @@ def occupancy_fuse(logodds, dims, box_min, box_max, pose, W, H, depth, uncertain
     _check(lib().r360_occupancy_fuse(d, lo, hi, fp(L), fp(p), W, H, fp(dep), None if unc is None else fp(unc)),
            "r360_occupancy_fuse")
     return L
+
+
+class Fusion:
+    """r360_fusion handle: the log-odds grid of Eq. 6 resident on the device between observations."""
+
+    def __init__(self, dims, box_min, box_max, logodds_init=None):
+        self._h = C.c_void_p()
+        d = (C.c_int32 * 3)(*[int(v) for v in dims])
+        lo = (C.c_float * 3)(*[float(v) for v in box_min])
+        hi = (C.c_float * 3)(*[float(v) for v in box_max])
+        self.N = d[0] * d[1] * d[2]
+        init = None
+        if logodds_init is not None:
+            keep = np.ascontiguousarray(logodds_init, np.float32).reshape(-1)
+            assert keep.size == self.N
+            init = keep.ctypes.data_as(C.POINTER(C.c_float))
+        _check(lib().r360_fusion_create(d, lo, hi, init, C.byref(self._h)), "r360_fusion_create")
+
+    def fuse(self, pose, W, H, depth, uncertainty=None):
+        """One observation; depth / uncertainty are numpy arrays (host) or torch CUDA float32 tensors (device)."""
+        p = np.ascontiguousarray(pose, np.float32).reshape(12)
+        pp = p.ctypes.data_as(C.POINTER(C.c_float))
+        if hasattr(depth, "is_cuda"):
+            assert depth.is_cuda and depth.is_contiguous() and depth.numel() == W * H
+            u = None if uncertainty is None else uncertainty.data_ptr()
+            _check(lib().r360_fusion_fuse_device(self._h, pp, W, H, depth.data_ptr(), u), "r360_fusion_fuse_device")
+            return
+        dep = np.ascontiguousarray(depth, np.float32).reshape(-1)
+        assert dep.size == W * H
+        unc = None if uncertainty is None else np.ascontiguousarray(uncertainty, np.float32).reshape(-1)
+        fp = lambda a: a.ctypes.data_as(C.POINTER(C.c_float))
+        _check(lib().r360_fusion_fuse(self._h, pp, W, H, fp(dep), None if unc is None else fp(unc)), "r360_fusion_fuse")
+
+    def read(self, occupancy=False):
+        """The log-odds grid (float32[N]); with occupancy=True also the thresholded uint8 grid (255 / 0)."""
+        L = np.empty(self.N, np.float32)
+        occ = np.empty(self.N, np.uint8) if occupancy else None
+        _check(lib().r360_fusion_read(self._h, L.ctypes.data_as(C.POINTER(C.c_float)),
+                                      None if occ is None else occ.ctypes.data_as(C.POINTER(C.c_uint8))), "r360_fusion_read")
+        return (L, occ) if occupancy else L
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib().r360_fusion_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def floorplan(occupancy, dims, occ_threshold, seed_xy, upper=None, lower=None):

@@ -65,7 +65,12 @@ __global__ void __launch_bounds__(1024) k_anchor(Voxels v, AssignState* st) {
     const uint32_t i = pos + threadIdx.x;
     if (i < v.S && v.label[i] < 0) atomicMin(&found, i);
     __syncthreads();
-    if (found != 0xFFFFFFFFu) break;
+    // every thread takes the window's result into a register and the block meets again before anyone starts the
+    // next window's atomicMin: a thread lagging behind this read could otherwise see a value of a later window
+    // (ADVICE round 1), and all threads leave the loop in the same iteration
+    const uint32_t f = found;
+    __syncthreads();
+    if (f != 0xFFFFFFFFu) break;
     pos += blockDim.x;
   }
   if (threadIdx.x == 0) {
@@ -176,6 +181,7 @@ extern "C" r360_status r360_assign_subfields(const int32_t dims[3], const float 
   const long long N = (long long)dims[0] * dims[1] * dims[2];
   std::vector<ushort4> coord;
   std::vector<long long> lin;
+  std::vector<int32_t> lab;               // (every host allocation inside the try: no exception crosses the C ABI)
   try {
     for (long long vox = 0; vox < N; ++vox) {
       labels_out[vox] = -1;
@@ -184,6 +190,7 @@ extern "C" r360_status r360_assign_subfields(const int32_t dims[3], const float 
                                    (unsigned short)(vox / ((long long)dims[0] * dims[1])), 0));
       lin.push_back(vox);
     }
+    lab.resize(coord.size());
   } catch (const std::bad_alloc&) { return R360_ERR_OOM; }
   const size_t S = coord.size();
   if ((size_t)n > S || S >= (1ull << kPosBits)) return R360_ERR_INVALID_ARG;
@@ -210,7 +217,6 @@ extern "C" r360_status r360_assign_subfields(const int32_t dims[3], const float 
     AssignState h{};
     h.q = (uint32_t)(S / (size_t)n);
     h.r = (uint32_t)(S % (size_t)n);
-    std::vector<int32_t> lab(S);
     A_CUDA(cudaStreamCreateWithFlags(&stream, cudaStreamNonBlocking));
     A_CUDA(cudaMalloc(&d_coord, S * sizeof(ushort4)));
     A_CUDA(cudaMalloc(&d_label, S * sizeof(int32_t)));

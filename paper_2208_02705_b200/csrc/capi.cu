@@ -88,10 +88,11 @@ size_t tc_smem_bytes(const NetShape& net);
 // Skip distances of the empty voxels (common.cuh: grid encoding): D = min(255, chessboard distance to
 // the nearest occupied voxel), by the two-pass 26-neighbour chamfer transform, which is exact for the
 // chessboard metric.  Occupied voxels (value < kEmptyBase) are left untouched.
-static void skip_distances(std::vector<uint16_t>& grid, const int dims[3]) {
+static bool skip_distances(std::vector<uint16_t>& grid, const int dims[3]) {
   const int Nx = dims[0], Ny = dims[1], Nz = dims[2];
   const size_t N = (size_t)Nx * Ny * Nz;
-  std::vector<uint8_t> dist(N);
+  std::vector<uint8_t> dist;
+  try { dist.resize(N); } catch (const std::bad_alloc&) { return false; }
   for (size_t v = 0; v < N; ++v) dist[v] = grid[v] < kEmptyBase ? 0 : 255;
   auto relax = [&](int z, int y, int x, int sgn) {
     // 13 neighbours that precede (sgn = -1) or follow (sgn = +1) the voxel in raster order
@@ -123,6 +124,7 @@ static void skip_distances(std::vector<uint16_t>& grid, const int dims[3]) {
       for (int x = Nx - 1; x >= 0; --x) relax(z, y, x, +1);
   for (size_t v = 0; v < N; ++v)
     if (grid[v] >= kEmptyBase) grid[v] = (uint16_t)(kEmptyBase | dist[v]);
+  return true;
 }
 
 extern "C" {
@@ -234,10 +236,11 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
       if (idx[a] > hi[(size_t)k * 3 + a]) hi[(size_t)k * 3 + a] = idx[a];
     }
   }
-  skip_distances(grid, g.dims);
+  if (!skip_distances(grid, g.dims)) return R360_ERR_OOM;
   for (long long i = 0; i < (long long)n * src.total; ++i)
     if (!std::isfinite(weights[i])) return R360_ERR_NONFINITE;
-  std::vector<SubfieldFrame> frames((size_t)n);
+  std::vector<SubfieldFrame> frames;
+  try { frames.resize((size_t)n); } catch (const std::bad_alloc&) { return R360_ERR_OOM; }
   for (int k = 0; k < n; ++k) {
     float c[3], ih[3];
     for (int a = 0; a < 3; ++a) {

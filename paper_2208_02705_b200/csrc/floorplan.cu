@@ -145,12 +145,17 @@ extern "C" r360_status r360_floorplan(const int32_t dims[3], const uint8_t* occu
     // F4 flood fill from the seed
     F_CUDA(cudaMemset(d_in, 0, n2));
     F_CUDA(cudaMemcpy(d_in + (size_t)seed_y * nx + seed_x, &one, 1, cudaMemcpyHostToDevice));
-    for (int it = 0; it < 4 * (nx + ny) + 8; ++it) {
-      int changed = 0;
-      F_CUDA(cudaMemset(d_changed, 0, sizeof(int)));
-      k_fill<<<fgrd, fblk>>>(d_a, nx, ny, d_in, d_changed);
-      F_CUDA(cudaMemcpy(&changed, d_changed, sizeof(int), cudaMemcpyDeviceToHost));
-      if (!changed) break;
+    // every launch relaxes each 32 x 32 tile to its local fixed point; a launch that changes anything adds at
+    // least one cell, so the fill ends after at most nx * ny launches -- it runs until nothing changes (a winding
+    // free region crosses tile borders far more often than any bound in nx + ny allows: ADVICE round 1)
+    {
+      int changed = 1;
+      for (size_t it = 0; changed; ++it) {
+        if (it > n2 + 8) { rc = R360_ERR_CUDA; goto done; }
+        F_CUDA(cudaMemset(d_changed, 0, sizeof(int)));
+        k_fill<<<fgrd, fblk>>>(d_a, nx, ny, d_in, d_changed);
+        F_CUDA(cudaMemcpy(&changed, d_changed, sizeof(int), cudaMemcpyDeviceToHost));
+      }
     }
     // F5-F7
     k_plan<<<grd, blk>>>(d_in, d_low, nx, ny, d_b);

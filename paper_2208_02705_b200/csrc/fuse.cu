@@ -12,6 +12,7 @@
 //   k_update : one thread per voxel applies Eq. 6 once and clears the flags
 // The result does not depend on the order of the rays (flags and a minimum), so it is reproducible bit for bit.
 #include <cmath>
+#include <new>
 #include <vector>
 
 #include "scene.h"
@@ -114,69 +115,166 @@ k_update(size_t N, float l_free, float* __restrict__ L, uint32_t* __restrict__ f
   umin[v] = 0x3F800000u;
 }
 
+__global__ void __launch_bounds__(256) k_fill_u32(uint32_t* __restrict__ p, size_t n, uint32_t v) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) p[i] = v;
+}
+
+// voxel occupied iff logit > ln(0.97 / 0.03) (reading O5): the uint8 occupancy of r360_scene_create
+__global__ void __launch_bounds__(256) k_threshold(const float* __restrict__ L, size_t n, float thr, uint8_t* __restrict__ occ) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) occ[i] = L[i] > thr ? 255 : 0;
+}
+
 }  // namespace
 
-extern "C" r360_status r360_occupancy_fuse(const int32_t dims[3], const float box_min[3], const float box_max[3],
-                                           float* logodds, const float pose[12], int32_t W, int32_t H,
-                                           const float* depth, const float* uncertainty) {
-  if (!dims || !box_min || !box_max || !logodds || !pose || !depth || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
-  if ((long long)W * H >= (1ll << 30)) return R360_ERR_INVALID_ARG;
-  GridParams g{};
+// The log-odds grid stays on the device between observations (Algorithm 1 stage I fuses T panoramas
+// progressively): no per-observation allocation, no grid crossing PCIe.
+struct r360_fusion {
+  r360::GridParams g{};
+  size_t N = 0;
+  float* d_L = nullptr;
+  uint32_t* d_flags = nullptr;        // kFree | kOcc of the observation being fused; zero between observations
+  uint32_t* d_umin = nullptr;         // bits of the smallest uncertainty per voxel; 1.0f between observations
+  float* d_tab = nullptr;             // trig tables of the last image size
+  int tab_W = 0, tab_H = 0;
+  float* d_pose = nullptr;
+  float* d_depth = nullptr;           // staging of host images
+  float* d_unc = nullptr;
+  size_t img_cap = 0;
+  uint8_t* d_occ = nullptr;           // r360_fusion_read: thresholded grid
+};
+
+extern "C" {
+
+void r360_fusion_destroy(r360_fusion* fu) {
+  if (!fu) return;
+  cudaFree(fu->d_L); cudaFree(fu->d_flags); cudaFree(fu->d_umin); cudaFree(fu->d_tab); cudaFree(fu->d_pose);
+  cudaFree(fu->d_depth); cudaFree(fu->d_unc); cudaFree(fu->d_occ);
+  cudaGetLastError();
+  delete fu;
+}
+
+r360_status r360_fusion_create(const int32_t dims[3], const float box_min[3], const float box_max[3],
+                               const float* logodds_init, r360_fusion** out) {
+  if (out) *out = nullptr;
+  if (!dims || !box_min || !box_max || !out) return R360_ERR_INVALID_ARG;
+  r360_fusion* fu = new (std::nothrow) r360_fusion();
+  if (!fu) return R360_ERR_OOM;
+  struct Guard {
+    r360_fusion* f;
+    ~Guard() { if (f) r360_fusion_destroy(f); }
+  } guard{fu};
   for (int a = 0; a < 3; ++a) {
     if (dims[a] < 1 || !(box_max[a] > box_min[a])) return R360_ERR_INVALID_ARG;
-    g.dims[a] = dims[a];
-    g.box_min[a] = box_min[a];
+    fu->g.dims[a] = dims[a];
+    fu->g.box_min[a] = box_min[a];
     volatile float ext = box_max[a] - box_min[a];               // voxel size exactly as the renderer computes it
-    g.vs[a] = ext / (float)dims[a];
-    g.inv_vs[a] = 1.0f / g.vs[a];
+    fu->g.vs[a] = ext / (float)dims[a];
+    fu->g.inv_vs[a] = 1.0f / fu->g.vs[a];
   }
+  if ((long long)dims[0] * dims[1] * dims[2] > (1ll << 31) - 1) return R360_ERR_INVALID_ARG;
+  const size_t N = fu->N = (size_t)dims[0] * dims[1] * dims[2];
+  R360_CUDA(cudaMalloc(&fu->d_L, N * sizeof(float)));
+  R360_CUDA(cudaMalloc(&fu->d_flags, N * sizeof(uint32_t)));
+  R360_CUDA(cudaMalloc(&fu->d_umin, N * sizeof(uint32_t)));
+  R360_CUDA(cudaMalloc(&fu->d_pose, 12 * sizeof(float)));
+  if (logodds_init) R360_CUDA(cudaMemcpy(fu->d_L, logodds_init, N * sizeof(float), cudaMemcpyHostToDevice));
+  else R360_CUDA(cudaMemset(fu->d_L, 0, N * sizeof(float)));
+  R360_CUDA(cudaMemset(fu->d_flags, 0, N * sizeof(uint32_t)));
+  k_fill_u32<<<(unsigned)((N + 255) / 256), 256>>>(fu->d_umin, N, 0x3F800000u);   // umin starts at 1.0
+  R360_CUDA(cudaGetLastError());
+  R360_CUDA(cudaDeviceSynchronize());
+  guard.f = nullptr;
+  *out = fu;
+  return R360_OK;
+}
+
+// depth / uncertainty: DEVICE pointers (for example the depth output of r360_render)
+r360_status r360_fusion_fuse_device(r360_fusion* fu, const float pose[12], int32_t W, int32_t H, const float* depth,
+                                    const float* uncertainty) {
+  if (!fu || !pose || !depth || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
+  if ((long long)W * H >= (1ll << 30)) return R360_ERR_INVALID_ARG;
   for (int i = 0; i < 12; ++i)
     if (!std::isfinite(pose[i])) return R360_ERR_INVALID_ARG;
-  const size_t N = (size_t)dims[0] * dims[1] * dims[2], R = (size_t)W * H;
-  // reading B2: trig of the pixel-centre angles in binary64, rounded once
-  const double kPi = 3.14159265358979323846;
-  std::vector<float> tab((size_t)2 * W + 2 * H);
-  for (int i = 0; i < W; ++i) {
-    const double phi = (((double)i + 0.5) - (double)W / 2.0) * (2.0 * kPi / (double)W);
-    tab[i] = (float)std::sin(phi);
-    tab[(size_t)W + i] = (float)std::cos(phi);
+  if (!fu->d_tab || fu->tab_W != W || fu->tab_H != H) {
+    // reading B2: trig of the pixel-centre angles in binary64, rounded once
+    const double kPi = 3.14159265358979323846;
+    std::vector<float> tab;
+    try { tab.resize((size_t)2 * W + 2 * H); } catch (const std::bad_alloc&) { return R360_ERR_OOM; }
+    for (int i = 0; i < W; ++i) {
+      const double phi = (((double)i + 0.5) - (double)W / 2.0) * (2.0 * kPi / (double)W);
+      tab[i] = (float)std::sin(phi);
+      tab[(size_t)W + i] = (float)std::cos(phi);
+    }
+    for (int j = 0; j < H; ++j) {
+      const double theta = -((((double)j + 0.5) - (double)H / 2.0) * (kPi / (double)H));
+      tab[(size_t)2 * W + j] = (float)std::sin(theta);
+      tab[(size_t)2 * W + H + j] = (float)std::cos(theta);
+    }
+    cudaFree(fu->d_tab);
+    fu->d_tab = nullptr;
+    R360_CUDA(cudaMalloc(&fu->d_tab, tab.size() * sizeof(float)));
+    R360_CUDA(cudaMemcpy(fu->d_tab, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice));
+    fu->tab_W = W;
+    fu->tab_H = H;
   }
-  for (int j = 0; j < H; ++j) {
-    const double theta = -((((double)j + 0.5) - (double)H / 2.0) * (kPi / (double)H));
-    tab[(size_t)2 * W + j] = (float)std::sin(theta);
-    tab[(size_t)2 * W + H + j] = (float)std::cos(theta);
-  }
-  float *d_L = nullptr, *d_tab = nullptr, *d_pose = nullptr, *d_depth = nullptr, *d_unc = nullptr;
-  uint32_t *d_flags = nullptr, *d_umin = nullptr;
-  r360_status rc = R360_OK;
-#define U_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { rc = r360_cuda_fail(e_, #call); goto done; } } while (0)
-  {
-    std::vector<uint32_t> ones(N, 0x3F800000u);                 // umin starts at 1.0
-    FrameParams f{};
-    U_CUDA(cudaMalloc(&d_L, N * sizeof(float)));
-    U_CUDA(cudaMalloc(&d_flags, N * sizeof(uint32_t)));
-    U_CUDA(cudaMalloc(&d_umin, N * sizeof(uint32_t)));
-    U_CUDA(cudaMalloc(&d_tab, tab.size() * sizeof(float)));
-    U_CUDA(cudaMalloc(&d_pose, 12 * sizeof(float)));
-    U_CUDA(cudaMalloc(&d_depth, R * sizeof(float)));
-    if (uncertainty) U_CUDA(cudaMalloc(&d_unc, R * sizeof(float)));
-    U_CUDA(cudaMemcpy(d_L, logodds, N * sizeof(float), cudaMemcpyHostToDevice));
-    U_CUDA(cudaMemset(d_flags, 0, N * sizeof(uint32_t)));
-    U_CUDA(cudaMemcpy(d_umin, ones.data(), N * sizeof(uint32_t), cudaMemcpyHostToDevice));
-    U_CUDA(cudaMemcpy(d_tab, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice));
-    U_CUDA(cudaMemcpy(d_pose, pose, 12 * sizeof(float), cudaMemcpyHostToDevice));
-    U_CUDA(cudaMemcpy(d_depth, depth, R * sizeof(float), cudaMemcpyHostToDevice));
-    if (uncertainty) U_CUDA(cudaMemcpy(d_unc, uncertainty, R * sizeof(float), cudaMemcpyHostToDevice));
-    f.W = W; f.H = H; f.ray0 = 0; f.pose0 = 0; f.pix0 = 0; f.n_rays = (unsigned)R; f.camera = 0;
-    f.poses = d_pose;
-    f.sin_phi = d_tab; f.cos_phi = d_tab + W; f.sin_theta = d_tab + 2 * (size_t)W; f.cos_theta = d_tab + 2 * (size_t)W + H;
-    k_mark<<<(unsigned)((R + 255) / 256), 256>>>(g, f, d_depth, d_unc, d_flags, d_umin);
-    k_update<<<(unsigned)((N + 255) / 256), 256>>>(N, (float)std::log(0.4 / 0.6), d_L, d_flags, d_umin);
-    U_CUDA(cudaGetLastError());
-    U_CUDA(cudaMemcpy(logodds, d_L, N * sizeof(float), cudaMemcpyDeviceToHost));
-  }
-done:
-#undef U_CUDA
-  cudaFree(d_L); cudaFree(d_flags); cudaFree(d_umin); cudaFree(d_tab); cudaFree(d_pose); cudaFree(d_depth); cudaFree(d_unc);
-  return rc;
+  R360_CUDA(cudaMemcpy(fu->d_pose, pose, 12 * sizeof(float), cudaMemcpyHostToDevice));
+  const size_t R = (size_t)W * H;
+  r360::FrameParams f{};
+  f.W = W; f.H = H; f.ray0 = 0; f.pose0 = 0; f.pix0 = 0; f.n_rays = (unsigned)R; f.camera = 0;
+  f.poses = fu->d_pose;
+  f.sin_phi = fu->d_tab; f.cos_phi = fu->d_tab + W;
+  f.sin_theta = fu->d_tab + 2 * (size_t)W; f.cos_theta = fu->d_tab + 2 * (size_t)W + H;
+  k_mark<<<(unsigned)((R + 255) / 256), 256>>>(fu->g, f, depth, uncertainty, fu->d_flags, fu->d_umin);
+  k_update<<<(unsigned)((fu->N + 255) / 256), 256>>>(fu->N, (float)std::log(0.4 / 0.6), fu->d_L, fu->d_flags, fu->d_umin);
+  R360_CUDA(cudaGetLastError());
+  return R360_OK;
 }
+
+// depth / uncertainty: HOST pointers
+r360_status r360_fusion_fuse(r360_fusion* fu, const float pose[12], int32_t W, int32_t H, const float* depth,
+                             const float* uncertainty) {
+  if (!fu || !pose || !depth || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
+  if ((long long)W * H >= (1ll << 30)) return R360_ERR_INVALID_ARG;
+  const size_t R = (size_t)W * H;
+  if (R > fu->img_cap) {
+    cudaFree(fu->d_depth); cudaFree(fu->d_unc);
+    fu->d_depth = fu->d_unc = nullptr;
+    fu->img_cap = 0;
+    R360_CUDA(cudaMalloc(&fu->d_depth, R * sizeof(float)));
+    R360_CUDA(cudaMalloc(&fu->d_unc, R * sizeof(float)));
+    fu->img_cap = R;
+  }
+  R360_CUDA(cudaMemcpy(fu->d_depth, depth, R * sizeof(float), cudaMemcpyHostToDevice));
+  if (uncertainty) R360_CUDA(cudaMemcpy(fu->d_unc, uncertainty, R * sizeof(float), cudaMemcpyHostToDevice));
+  return r360_fusion_fuse_device(fu, pose, W, H, fu->d_depth, uncertainty ? fu->d_unc : nullptr);
+}
+
+r360_status r360_fusion_read(r360_fusion* fu, float* logodds_out, uint8_t* occupancy_out) {
+  if (!fu || (!logodds_out && !occupancy_out)) return R360_ERR_INVALID_ARG;
+  if (logodds_out) R360_CUDA(cudaMemcpy(logodds_out, fu->d_L, fu->N * sizeof(float), cudaMemcpyDeviceToHost));
+  if (occupancy_out) {
+    if (!fu->d_occ) R360_CUDA(cudaMalloc(&fu->d_occ, fu->N));
+    k_threshold<<<(unsigned)((fu->N + 255) / 256), 256>>>(fu->d_L, fu->N, (float)std::log(0.97 / 0.03), fu->d_occ);
+    R360_CUDA(cudaGetLastError());
+    R360_CUDA(cudaMemcpy(occupancy_out, fu->d_occ, fu->N, cudaMemcpyDeviceToHost));
+  }
+  return R360_OK;
+}
+
+// one observation on a host grid: create, fuse, read, destroy
+r360_status r360_occupancy_fuse(const int32_t dims[3], const float box_min[3], const float box_max[3],
+                                float* logodds, const float pose[12], int32_t W, int32_t H,
+                                const float* depth, const float* uncertainty) {
+  if (!dims || !box_min || !box_max || !logodds || !pose || !depth || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
+  r360_fusion* fu = nullptr;
+  r360_status st = r360_fusion_create(dims, box_min, box_max, logodds, &fu);
+  if (st != R360_OK) return st;
+  st = r360_fusion_fuse(fu, pose, W, H, depth, uncertainty);
+  if (st == R360_OK) st = r360_fusion_read(fu, logodds, nullptr);
+  r360_fusion_destroy(fu);
+  return st;
+}
+
+}  // extern "C"

@@ -390,7 +390,7 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
       pd.next = 0;
       return st;
     }
-    pd.chunks.push_back({job.ray0, job.n_rays, job.out0});
+    pd.chunks.push_back({job.ray0, job.n_rays, job.out0});   // (capacity reserved above: cannot throw)
     if (exact) pd.next = chunk_idx + 1;                        // nothing to verify
     if (host_rgb) enqueue_host_copy(sc, pd, job);
     if (!cap && !exact && (st = r360_settle(sc, false)) != R360_OK) return st;   // earlier chunks, without waiting

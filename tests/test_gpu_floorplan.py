@@ -62,6 +62,27 @@ def test_baseline_scenes(r360, config):
     assert np.array_equal(got2, ref2)
 
 
+def test_winding_region_is_filled_completely(r360):
+    """A serpentine of 300 corridors on a 1200 x 1200 grid: the free region crosses 32 x 32 tile borders about
+    11 000 times, more than the 4 (nx + ny) + 8 launches the flood fill used to stop after."""
+    from oracle.floorplan import INTERIOR, floorplan
+    nx = ny = 1200
+    nz = 4
+    occ = np.full((nz, ny, nx), 5, np.uint8)
+    occ[:, 0, :] = occ[:, -1, :] = 250
+    occ[:, :, 0] = occ[:, :, -1] = 250
+    for k, x in enumerate(range(4, nx - 4, 4)):          # walls one cell thick, corridors three cells wide
+        occ[:, :, x] = 250
+        if k % 2 == 0:
+            occ[:, ny - 4:ny - 1, x] = 5                  # door at the far end ...
+        else:
+            occ[:, 1:4, x] = 5                            # ... then at the near end
+    ref = floorplan(occ, (nx, ny, nz), 248, (2, 2))
+    got = r360.floorplan(occ, (nx, ny, nz), 248, (2, 2))
+    assert np.array_equal(got, ref)
+    assert (ref[:, nx - 3] & INTERIOR).any()              # the fill reached the last corridor
+
+
 def test_errors(r360):
     occ = np.full((4, 6, 6), 255, np.uint8)
     with pytest.raises(r360.R360Error):

@@ -95,3 +95,55 @@ def test_recovers_the_scene_from_its_own_depth(r360, oracle):
     assert (L[first_hits] > 0).all()                          # everything the first pose saw carries occupied evidence
     assert (L[~occ] <= 0).all()
     ora.close()
+
+
+def test_resident_grid_equals_repeated_single_observations(r360, oracle):
+    """r360_fusion_*: the grid stays on the device over a sequence of observations; the result equals the oracle's
+    observation-by-observation fusion bit for bit, and the thresholded occupancy is reading O5."""
+    from oracle.fusion import L_OCC_THRESHOLD, fuse
+    rng = np.random.default_rng(4)
+    dims, bmin, bmax = (24, 18, 10), (-2.0, -1.5, -1.0), (2.1, 1.4, 0.9)
+    W, H = 80, 40
+    R0 = np.array([[0, 0, 1], [-1, 0, 0], [0, -1, 0]], np.float64)
+    fu = r360.Fusion(dims, bmin, bmax)
+    Lo = np.zeros(dims[0] * dims[1] * dims[2], np.float32)
+    for k in range(5):
+        yaw = rng.uniform(0, 6.28)
+        c, s = np.cos(yaw), np.sin(yaw)
+        R = np.array([[c, -s, 0], [s, c, 0], [0, 0, 1]]) @ R0
+        pose = np.concatenate([R, rng.uniform(-0.4, 0.4, 3)[:, None]], 1).astype(np.float32).reshape(12)
+        depth = rng.uniform(0.3, 2.5, (H, W)).astype(np.float32)
+        unc = rng.uniform(0, 1, (H, W)).astype(np.float32) if k % 2 else None
+        fu.fuse(pose, W, H, depth, unc)
+        Lo = fuse(oracle, Lo, dims, bmin, bmax, pose, W, H, depth, unc)
+    Lg, occ = fu.read(occupancy=True)
+    assert _eq(Lg, Lo)
+    assert np.array_equal(occ, np.where(Lo > np.float32(L_OCC_THRESHOLD), 255, 0).astype(np.uint8))
+    # an initial grid, and a second image size on the same handle
+    fu2 = r360.Fusion(dims, bmin, bmax, logodds_init=Lo)
+    depth = rng.uniform(0.3, 2.5, (33, 70)).astype(np.float32)
+    fu2.fuse(pose, 70, 33, depth)
+    assert _eq(fu2.read(), fuse(oracle, Lo, dims, bmin, bmax, pose, 70, 33, depth))
+    fu.close()
+    fu2.close()
+
+
+def test_fusion_fed_by_the_renderers_own_depth(r360, oracle):
+    """the renderer's depth output (a DEVICE buffer, Eq. 4's radial distance) goes straight into
+    the fusion (r360_fusion_fuse_device) -- the synthetic stand-in for 360NeRF's depth panoramas.  Same grid as
+    fusing the image after a round trip through the host."""
+    from oracle.fusion import fuse
+    sc = get_scene(1)
+    gpu = r360.scene_from(sc)
+    W, H = 128, 64
+    rgb, depth = gpu.render(sc.poses[0], W, H)
+    import torch
+    torch.cuda.synchronize()
+    fu = r360.Fusion(sc.dims, sc.box_min, sc.box_max)
+    fu.fuse(sc.poses[0], W, H, depth.contiguous())
+    ref = fuse(oracle, np.zeros(int(np.prod(sc.dims)), np.float32), sc.dims, sc.box_min, sc.box_max, sc.poses[0], W, H,
+               depth.cpu().numpy())
+    assert _eq(fu.read(), ref)
+    assert (ref != 0).sum() > 1000
+    fu.close()
+    gpu.close()
