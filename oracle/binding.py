@@ -23,7 +23,8 @@ def build_oracle(force: bool = False) -> str:
     if (not force and os.path.exists(_SO)
             and os.path.getmtime(_SO) >= max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))):
         return _SO
-    subprocess.check_call(["gcc", *CFLAGS, "-o", _SO, _SRC, "-lm"])
+    # R360_ORACLE_CFLAGS: extra flags, e.g. "-fsanitize=address,undefined -g" for a sanitizer run of the CPU tests
+    subprocess.check_call(["gcc", *CFLAGS, *os.environ.get("R360_ORACLE_CFLAGS", "").split(), "-o", _SO, _SRC, "-lm"])
     return _SO
 
 

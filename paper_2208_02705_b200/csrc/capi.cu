@@ -5,6 +5,7 @@
 #include <cstring>
 #include <limits>
 #include <new>
+#include <thread>
 #include <vector>
 
 #include "scene.h"
@@ -85,45 +86,49 @@ bool tc_pack_subfield(const NetShape& net, const float* src_blob, void* dst, int
 size_t tc_smem_bytes(const NetShape& net);
 }  // namespace r360
 
-// Skip distances of the empty voxels (common.cuh: grid encoding): D = min(255, chessboard distance to
-// the nearest occupied voxel), by the two-pass 26-neighbour chamfer transform, which is exact for the
-// chessboard metric.  Occupied voxels (value < kEmptyBase) are left untouched.
-static bool skip_distances(std::vector<uint16_t>& grid, const int dims[3]) {
+// Octant skip distances of the empty voxels (common.cuh): for the octant with direction signs (sx, sy, sz),
+//   D(v) = 0 if v is occupied, else min(255, 1 + min over the 7 neighbours v + (ex sx, ey sy, ez sz), e in {0,1}^3 \ 0,
+//   of D(neighbour)), a neighbour outside the grid counting as 255
+// -- the cube of D voxels per axis that starts at v and extends in the octant's direction is empty iff v is empty
+// and the seven cubes of D-1 voxels that start at those neighbours are.  One sweep per octant, against the
+// direction of travel, so that every neighbour is final when it is read; the eight sweeps run on eight threads.
+static bool skip_distances(const std::vector<uint16_t>& grid, const int dims[3], std::vector<uint8_t>& skip) {
   const int Nx = dims[0], Ny = dims[1], Nz = dims[2];
   const size_t N = (size_t)Nx * Ny * Nz;
-  std::vector<uint8_t> dist;
-  try { dist.resize(N); } catch (const std::bad_alloc&) { return false; }
-  for (size_t v = 0; v < N; ++v) dist[v] = grid[v] < kEmptyBase ? 0 : 255;
-  auto relax = [&](int z, int y, int x, int sgn) {
-    // 13 neighbours that precede (sgn = -1) or follow (sgn = +1) the voxel in raster order
-    uint8_t& c = dist[((size_t)z * Ny + y) * Nx + x];
-    int m = c;
-    if (m == 0) return;
-    for (int dz = 0; dz <= 1; ++dz) {
-      const int z2 = z + sgn * dz;
-      if (z2 < 0 || z2 >= Nz) continue;
-      for (int dy = (dz ? -1 : 0); dy <= 1; ++dy) {
-        const int y2 = y + sgn * dy;
-        if (y2 < 0 || y2 >= Ny) continue;
-        for (int dx = ((dz || dy) ? -1 : 1); dx <= 1; ++dx) {
-          const int x2 = x + sgn * dx;
-          if (x2 < 0 || x2 >= Nx) continue;
-          const int nb = dist[((size_t)z2 * Ny + y2) * Nx + x2] + 1;
-          if (nb < m) m = nb;
+  try { skip.assign(N * 8, 0); } catch (const std::bad_alloc&) { return false; }
+  auto sweep = [&](int o) {
+    const int sx = (o & 1) ? -1 : 1, sy = (o & 2) ? -1 : 1, sz = (o & 4) ? -1 : 1;
+    auto at = [&](int x, int y, int z) -> int {
+      if (x < 0 || x >= Nx || y < 0 || y >= Ny || z < 0 || z >= Nz) return 255;
+      return skip[(((size_t)z * Ny + y) * Nx + x) * 8 + o];
+    };
+    for (int kz = 0; kz < Nz; ++kz) {
+      const int z = sz > 0 ? Nz - 1 - kz : kz;
+      for (int ky = 0; ky < Ny; ++ky) {
+        const int y = sy > 0 ? Ny - 1 - ky : ky;
+        for (int kx = 0; kx < Nx; ++kx) {
+          const int x = sx > 0 ? Nx - 1 - kx : kx;
+          const size_t v = ((size_t)z * Ny + y) * Nx + x;
+          if (grid[v] < kEmptyBase) { skip[v * 8 + o] = 0; continue; }
+          int m = 255;
+          for (int e = 1; e < 8; ++e) {
+            const int nb = at(x + ((e & 1) ? sx : 0), y + ((e & 2) ? sy : 0), z + ((e & 4) ? sz : 0));
+            if (nb < m) m = nb;
+          }
+          skip[v * 8 + o] = (uint8_t)(m >= 254 ? 255 : m + 1);
         }
       }
     }
-    c = (uint8_t)m;
   };
-  // forward scan uses the neighbours already visited (sgn = -1), backward scan the others
-  for (int z = 0; z < Nz; ++z)
-    for (int y = 0; y < Ny; ++y)
-      for (int x = 0; x < Nx; ++x) relax(z, y, x, -1);
-  for (int z = Nz - 1; z >= 0; --z)
-    for (int y = Ny - 1; y >= 0; --y)
-      for (int x = Nx - 1; x >= 0; --x) relax(z, y, x, +1);
-  for (size_t v = 0; v < N; ++v)
-    if (grid[v] >= kEmptyBase) grid[v] = (uint16_t)(kEmptyBase | dist[v]);
+  // the eight sweeps write disjoint bytes; whatever could not get a thread runs here
+  std::thread th[8];
+  int started = 0;
+  try {
+    for (; started < 7; ++started) th[started] = std::thread(sweep, started);
+  } catch (...) {
+  }
+  for (int o = started; o < 8; ++o) sweep(o);
+  for (int o = 0; o < started; ++o) th[o].join();
   return true;
 }
 
@@ -155,7 +160,7 @@ int64_t r360_params_per_subfield(const r360_scene_desc* desc) {
 
 void r360_scene_destroy(r360_scene* sc) {
   if (!sc) return;
-  cudaFree(sc->d_grid); cudaFree(sc->d_frames); cudaFree(sc->d_wt); cudaFree(sc->d_wpack); cudaFree(sc->d_wpack_f16);
+  cudaFree(sc->d_grid); cudaFree(sc->d_skip); cudaFree(sc->d_frames); cudaFree(sc->d_wt); cudaFree(sc->d_wpack); cudaFree(sc->d_wpack_f16);
   cudaFree(sc->d_tables); cudaFree(sc->d_poses);
   cudaFree(sc->buf.ray_cnt); cudaFree(sc->buf.ray_off); cudaFree(sc->buf.block_sum);
   cudaFree(sc->buf.bin_cnt); cudaFree(sc->buf.bin_start); cudaFree(sc->buf.bin_cursor);
@@ -225,7 +230,7 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
     hi.assign((size_t)n * 3, -1);
   } catch (const std::bad_alloc&) { return R360_ERR_OOM; }
   for (long long v = 0; v < N; ++v) {
-    if (occupancy[v] < desc->occ_threshold) { grid[(size_t)v] = (uint16_t)(kEmptyBase | 0xFFu); continue; }
+    if (occupancy[v] < desc->occ_threshold) { grid[(size_t)v] = (uint16_t)0xFFFFu; continue; }
     int k = voxel_subfield[v];
     if (k < 0 || k >= n) return R360_ERR_BAD_LABEL;
     grid[(size_t)v] = (uint16_t)k;
@@ -236,7 +241,8 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
       if (idx[a] > hi[(size_t)k * 3 + a]) hi[(size_t)k * 3 + a] = idx[a];
     }
   }
-  if (!skip_distances(grid, g.dims)) return R360_ERR_OOM;
+  std::vector<uint8_t> skip;
+  if (!skip_distances(grid, g.dims, skip)) return R360_ERR_OOM;
   for (long long i = 0; i < (long long)n * src.total; ++i)
     if (!std::isfinite(weights[i])) return R360_ERR_NONFINITE;
   std::vector<SubfieldFrame> frames;
@@ -298,6 +304,9 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
   R360_CUDA(cudaMalloc(&sc->d_frames, (size_t)n * sizeof(SubfieldFrame)));
   R360_CUDA(cudaMalloc(&sc->d_wt, wt.size() * sizeof(float)));
   R360_CUDA(cudaMemcpy(sc->d_grid, grid.data(), (size_t)N * sizeof(uint16_t), cudaMemcpyHostToDevice));
+  R360_CUDA(cudaMalloc(&sc->d_skip, skip.size()));
+  R360_CUDA(cudaMemcpy(sc->d_skip, skip.data(), skip.size(), cudaMemcpyHostToDevice));
+  sc->grid_p.skip = sc->d_skip;
   R360_CUDA(cudaMemcpy(sc->d_frames, frames.data(), (size_t)n * sizeof(SubfieldFrame), cudaMemcpyHostToDevice));
   R360_CUDA(cudaMemcpy(sc->d_wt, wt.data(), wt.size() * sizeof(float), cudaMemcpyHostToDevice));
   if (!wpack.empty()) {

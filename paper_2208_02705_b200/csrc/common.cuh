@@ -6,10 +6,15 @@
 
 namespace r360 {
 
-// Fused occupancy + label + skip-distance grid (uint16 per voxel):
+// Fused occupancy + label grid (uint16 per voxel):
 //   value <  kEmptyBase : occupied, the value is the subfield label
-//   value >= kEmptyBase : empty, low byte = D = min(255, chessboard distance in voxels to the nearest
-//                         occupied voxel) >= 1, i.e. the cube of half-size D-1 around the voxel is empty
+//   value >= kEmptyBase : empty
+// and, beside it, the skip distances of the empty voxels, ONE PER OCTANT of ray directions (uint8[N][8], octant
+// o = [d_x < 0] + 2 [d_y < 0] + 4 [d_z < 0]): skip[v][o] = min(255, largest D such that the cube of D voxels per axis
+// that starts at v and extends in the octant's direction holds no occupied voxel) >= 1 for an empty v.  A ray only
+// ever moves forward on every axis, so this one-sided cube is all it can reach before it leaves it -- and it is far
+// larger than a cube centred on v (next to a wall a ray that leaves the wall jumps the whole room, where the
+// distance to the NEAREST occupied voxel is 1).
 constexpr uint32_t kEmptyBase = 0xFF00u;
 constexpr int kMaxSubfields = 0xFF00;
 constexpr int kTileRows = 128;              // rows (samples) per MLP tile
@@ -21,6 +26,7 @@ struct GridParams {
   float box_min[3];
   float vs[3];           // voxel size per axis: (box_max - box_min) / dims, binary32 (reading C)
   float inv_vs[3];       // 1 / vs: only for index GUESSES that are then verified against the planes
+  const uint8_t* skip;   // device, [N][8]: octant skip distances of the empty voxels (above); null = no skipping
   int K;                 // samples per occupied voxel crossed (reading D)
   float Kf;
   float Kinv;            // 1 / K when K is a power of two (x * Kinv is then x / K bit for bit), else 0
@@ -117,11 +123,11 @@ __device__ __forceinline__ float plane(const GridParams& g, int a, int k) {
 //
 // Reading C5: the crossed set is a per-voxel predicate, max(t0, max_a tn_a(i)) < min_a tf_a(i), with
 // every distance computed from the voxel index through t_at(); it does not depend on the path taken.
-// So from an empty voxel whose skip distance is D the walk leaves the whole empty cube of half-size
-// r = D-1 at once: the exit distance `to` is the smallest far-plane distance of the CUBE, the axis of
-// the minimum steps to the voxel behind that plane, and on the other two axes the new index is the
-// first one (along the ray) whose far plane lies beyond `to` -- found from a position guess and then
-// verified against the planes themselves, so no rounding of the guess can change the result.
+// So from an empty voxel whose skip distance (for the ray's octant) is D the walk leaves the whole empty
+// cube [idx, idx + (D-1) step] at once: the exit distance `to` is the smallest far-plane distance of the
+// CUBE, the axis of the minimum steps to the voxel behind that plane, and on the other two axes the new
+// index is the first one (along the ray) whose far plane lies beyond `to` -- found from a position guess
+// and then verified against the planes themselves, so no rounding of the guess can change the result.
 // The entry distance of the next voxel is max(t0, to, its near planes), which is exactly the
 // oracle's max(t0, tn_x, tn_y, tn_z); for a plain one-voxel step this reduces to max(ti, to).
 struct Walker {
@@ -129,6 +135,7 @@ struct Walker {
   float t0, ti;     // clip distance; entry distance of the current voxel
   int idx[3];
   int step[3], off[3];   // direction of travel per axis: step = +1 / -1, off = 1 / 0 (index offset of the far plane)
+  int octant;            // [d_x < 0] + 2 [d_y < 0] + 4 [d_z < 0]: which skip distance of a voxel this ray uses
   bool par[3];
   bool alive;
 
@@ -138,6 +145,7 @@ struct Walker {
 
   __device__ __forceinline__ void init(const GridParams& g, const Ray& ray) {
     alive = true;
+    octant = 0;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       o[a] = ray.o[a];
@@ -145,6 +153,7 @@ struct Walker {
       par[a] = fabsf(ray.d[a]) < kParallelEps;
       off[a] = ray.d[a] < 0.0f ? 0 : 1;
       step[a] = 2 * off[a] - 1;
+      octant |= (1 - off[a]) << a;
       inv[a] = par[a] ? 0.0f : __fdiv_rn(1.0f, ray.d[a]);
     }
     // C2: clip against the box
@@ -184,10 +193,13 @@ struct Walker {
   __device__ __forceinline__ bool advance(const GridParams& g, const uint16_t* __restrict__ grid,
                                        uint32_t& lab, float& t_in, float& t_out) {
     {
-      const uint32_t l = __ldg(grid + (idx[2] * g.dims[1] + idx[1]) * g.dims[0] + idx[0]);
+      // (unsigned index arithmetic: one multiply-add per level and a 32-bit offset)
+      const uint32_t lin = ((uint32_t)idx[2] * (uint32_t)g.dims[1] + (uint32_t)idx[1]) * (uint32_t)g.dims[0] + (uint32_t)idx[0];
+      const uint32_t l = __ldg(grid + lin);
+      const uint32_t sk = __ldg(g.skip + (size_t)lin * 8u + (uint32_t)octant);   // requested with the grid word
       const bool empty = l >= kEmptyBase;
-      const int r = empty ? (int)(l & 0xFFu) - 1 : 0;     // half-size of the empty cube (0: this voxel only)
-      // far planes of the cube [idx - r, idx + r], clamped to the grid
+      const int r = empty ? (int)sk - 1 : 0;     // the cube [idx, idx + r step] is empty (0: this voxel only)
+      // far planes of that cube, clamped to the grid
       int kx[3];
       float tf[3];
 #pragma unroll
@@ -215,8 +227,9 @@ struct Walker {
 #pragma unroll
         for (int a = 0; a < 3; ++a) {
           if (a != amin && !par[a] && alive) {
-            const int lo = max(idx[a] - r, 0), hi = min(idx[a] + r, g.dims[a] - 1);
-            const int first = off[a] ? lo : hi;
+            // the ray only moves forward: its index on this axis lies between idx and idx + r step
+            const int lo = off[a] ? idx[a] : max(idx[a] - r, 0), hi = off[a] ? min(idx[a] + r, g.dims[a] - 1) : idx[a];
+            const int first = idx[a];
             const float p = __fmaf_rn(to, d[a], o[a]);
             int gi = __float2int_rd((p - g.box_min[a]) * g.inv_vs[a]);     // guess, verified below
             gi = min(max(gi, lo), hi);

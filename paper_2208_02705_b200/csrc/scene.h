@@ -13,7 +13,8 @@ struct r360_scene {
   int n_sms = 148;
   int segs_per_tile = 16;
   // scene-constant device data
-  uint16_t* d_grid = nullptr;               // fused occupancy + label + skip distance (common.cuh)
+  uint16_t* d_grid = nullptr;               // fused occupancy + label (common.cuh)
+  uint8_t* d_skip = nullptr;                // [N][8] octant skip distances of the empty voxels (common.cuh)
   r360::SubfieldFrame* d_frames = nullptr;  // [n]
   float* d_wt = nullptr;                    // [n * lay.total] fp32, transposed + padded
   void* d_wpack = nullptr;                  // [n * wpack_stride] bfloat16 operand tiles + fp32 head biases
