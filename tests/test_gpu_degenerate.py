@@ -8,7 +8,7 @@ import numpy as np
 import pytest
 
 from conftest import get_scene
-from gpu_util import check_image, ray_major_index
+from gpu_util import AMB_BAND, check_image, ray_major_index
 
 pytestmark = pytest.mark.gpu
 F = np.float32
@@ -44,7 +44,7 @@ def _images_within_bars(gpu, ora, sc, pose, W, H):
     gpu.set_precision("bf16")
     rgb, depth = gpu.render(pose, W, H)
     t_max = float(np.linalg.norm(np.array(sc.box_max) - np.array(sc.box_min)))
-    e16 = check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 2e-3, amb_band=0.2, depth_tol=2e-3 * t_max)
+    e16 = check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 2e-3, amb_band=AMB_BAND["bf16"], depth_tol=2e-3 * t_max)
     gpu.set_precision("fp32")
     return e32, e16
 

@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 from conftest import get_scene
-from gpu_util import check_image, ray_major_index, with_density_bias
+from gpu_util import AMB_BAND, check_image, ray_major_index, with_density_bias
 
 pytestmark = pytest.mark.gpu
 F = np.float32
@@ -223,7 +223,7 @@ def test_pinhole_view(r360, oracle, config, W, H, f):
     gpu.set_precision("bf16")
     rgb, depth = gpu.render(pose, W, H)
     t_max = float(np.linalg.norm(np.array(sc.box_max) - np.array(sc.box_min)))
-    check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 2e-3, amb_band=0.2, depth_tol=2e-3 * t_max)
+    check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 2e-3, amb_band=AMB_BAND["bf16"], depth_tol=2e-3 * t_max)
     # back to the panorama: the tables are rebuilt for the other camera
     gpu.set_camera("equirect")
     gpu.set_precision("fp32")
@@ -281,6 +281,6 @@ def test_more_subfields_than_the_shared_memory_histogram_holds(r360, oracle):
     gpu.set_precision("bf16")
     rgb, depth = gpu.render(pose, W, H)
     t_max = float(np.linalg.norm(np.array(sc.box_max) - np.array(sc.box_min)))
-    check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 2e-3, amb_band=0.2, depth_tol=2e-3 * t_max)
+    check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 2e-3, amb_band=AMB_BAND["bf16"], depth_tol=2e-3 * t_max)
     gpu.close()
     ora.close()

@@ -6,7 +6,7 @@ import numpy as np
 import pytest
 
 from conftest import get_scene
-from gpu_util import check_image, with_density_bias
+from gpu_util import AMB_BAND, check_image, with_density_bias
 
 pytestmark = pytest.mark.gpu
 F = np.float32
@@ -27,8 +27,9 @@ def _t_max(sc):
     return float(np.linalg.norm(np.array(sc.box_max) - np.array(sc.box_min)))
 
 
-def _cmp(r360, oracle, sc, weights=None, amb_band=0.2, px=None, py=None, tol=TOL, precision="bf16", pose=None,
+def _cmp(r360, oracle, sc, weights=None, amb_band=None, px=None, py=None, tol=TOL, precision="bf16", pose=None,
          **desc_over):
+    amb_band = AMB_BAND[precision] if amb_band is None else amb_band
     over = dict(desc_over)
     if weights is not None:
         over["weights"] = weights
@@ -107,37 +108,36 @@ def test_render_tc_width64(r360, oracle, prec):
     _cmp(r360, oracle, sc, weights=w, hidden_width=64, n_hidden=3, precision=prec)
 
 
-def test_render_bf16_early_out(r360, oracle, scene1):
-    # Stress scene, NOT one of BASELINE.json's configs: density bias 40 makes every pixel the colour of
-    # its first one or two samples (alpha ~ 0.7 per sample), so the per-sample bf16 error of the colour
-    # head (measured <= 2.4e-3) is not averaged over tens of samples as it is in the configs the 2e-3 bar
-    # is stated for.  Bound used here: 4e-3.  The stopping sample depends
-    # on sigma (bf16-perturbed): rays whose T passes within 20 % of tau may stop one sample earlier or
-    # later (reading G4, widened for bf16).
-    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 40.0), amb_band=0.2,
-                             tol=4e-3)
+BF16_SINGLE_SAMPLE_BOUND = 4e-3
+
+
+def test_bfloat16_operands_on_opaque_scenes_stay_within_their_format_limit(r360, oracle, scene1):
+    """NOT a north_star claim: a characterisation of mode 1 (bfloat16 operands) on scenes whose pixels are the colour
+    of their first one or two samples (density bias 40; density beyond binary16's range, stored clamped to 65504).
+    A sample's colour through five layers of 8-bit-significand operands is off by up to 2.7e-3
+    (tests/test_rounding_budget.py: weights and activations contribute equally, no layer dominates), and with one
+    sample per pixel nothing averages it out: measured 2.4e-3 / 2.6e-3 here, above north_star's 2e-3.  The bound
+    asserted is that format limit with margin, 4e-3; the mode that meets 2e-3 on these scenes is binary16 operands
+    (test_render_f16_opaque_scenes below: 3.3e-4 / 4.5e-4).  On all five BASELINE.json configs, where a pixel
+    averages 35-290 samples, mode 1 is within 2e-3 (tests above and below)."""
+    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 40.0), tol=BF16_SINGLE_SAMPLE_BOUND)
     print("dense stress bf16 max rgb err", e_rgb)
-
-
-@pytest.mark.parametrize("act", [0, 1])
-def test_render_bf16_saturating_density(r360, oracle, scene1, act):
-    # density far beyond binary16's range: the tensor path stores sigma as binary16 clamped to 65504, alpha is 1
-    # either way, so every pixel is the colour of its first sample (per-sample bf16 error: the 4e-3 bound above)
-    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 1.0e6), amb_band=0.2,
-                             tol=4e-3, density_activation=act)
-    print("saturating density bf16 max rgb err", e_rgb)
+    for act in (0, 1):
+        e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 1.0e6),
+                                 tol=BF16_SINGLE_SAMPLE_BOUND, density_activation=act)
+        print("saturating density bf16 act", act, "max rgb err", e_rgb)
 
 
 def test_render_f16_opaque_scenes(r360, oracle, scene1):
     """The scene class the method is for (trained scenes: opaque surfaces end rays early) at
     north_star's bar, 2e-3, on the binary16-operand tensor path: density bias 40 (every pixel is the colour of its
     first one or two samples) and density far beyond binary16's range (sigma stored clamped to 65504, alpha = 1).
-    Ambiguity band 0.02: |dT/T| <= ln(1/tau) * max relative error of sigma = 6.9 * 2e-3."""
-    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 40.0), amb_band=0.02,
+    Ambiguity band: gpu_util.AMB_BAND."""
+    e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 40.0),
                              tol=TOL, precision="f16")
     print("dense stress f16 max rgb err", e_rgb, "ambiguous", n_amb)
     for act in (0, 1):
-        e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 1.0e6), amb_band=0.02,
+        e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 1.0e6),
                                  tol=TOL, density_activation=act, precision="f16")
         print("saturating density f16 act", act, "max rgb err", e_rgb)
 
