@@ -166,7 +166,7 @@ void r360_scene_destroy(r360_scene* sc) {
   cudaFree(sc->buf.bin_cnt); cudaFree(sc->buf.bin_start); cudaFree(sc->buf.bin_cursor);
   cudaFree(sc->buf.tile_start); cudaFree(sc->buf.totals);
   cudaDeviceSynchronize();   // (work of the last calls may still use the buffers)
-  cudaFree(sc->buf.seg_tin); cudaFree(sc->buf.seg_dt); cudaFree(sc->buf.recs); cudaFree(sc->buf.out);
+  cudaFree(sc->buf.seg_td); cudaFree(sc->buf.recs); cudaFree(sc->buf.out);
   cudaFree(sc->d_dirblk);
   cudaFree(sc->buf.hit_t); cudaFree(sc->buf.hit_lab);
   cudaFree(sc->buf.bin_ovf); cudaFree(sc->buf.blk_list); cudaFree(sc->buf.blk_list_n);

@@ -14,6 +14,22 @@ __device__ __forceinline__ float4 unpack_half4(uint2 q) {
   return make_float4(a.x, a.y, c.x, c.y);
 }
 
+__device__ __forceinline__ void write_pixel(const FrameParams& f, void* out_rgb, void* out_depth, size_t gr, float C0,
+                                            float C1, float C2, float D) {
+  if (f.out_format == 0) {
+    float* o = reinterpret_cast<float*>(out_rgb) + gr * 3;
+    o[0] = C0; o[1] = C1; o[2] = C2;
+    reinterpret_cast<float*>(out_depth)[gr] = D;
+  } else {
+    // R360_OUT_RGB8_D16: colour rounded to the nearest of 256 levels, depth to binary16
+    uint8_t* o = reinterpret_cast<uint8_t*>(out_rgb) + gr * 3;
+    o[0] = (uint8_t)__float2int_rn(__saturatef(C0) * 255.0f);
+    o[1] = (uint8_t)__float2int_rn(__saturatef(C1) * 255.0f);
+    o[2] = (uint8_t)__float2int_rn(__saturatef(C2) * 255.0f);
+    reinterpret_cast<__half*>(out_depth)[gr] = __float2half_rn(D);
+  }
+}
+
 // Tensor path, KK samples of 8 bytes per segment (KK even: whole 16-byte words): the NEXT segment's samples are
 // requested before this one's are composited, so two segments are in flight per ray.
 template <int KK>
@@ -23,15 +39,17 @@ __device__ __forceinline__ void composite_half_segments(const ChunkBuffers& b, u
   constexpr int Q = KK / 2;
   const uint4* o = reinterpret_cast<const uint4*>(reinterpret_cast<const uint2*>(b.out) + (size_t)off * KK);
   uint4 q[Q], qn[Q];
-  float t_in = b.seg_tin[off], dt = b.seg_dt[off], t_in_n = 0.f, dt_n = 0.f;
+  const float2 td0 = b.seg_td[off];
+  float t_in = td0.x, dt = td0.y, t_in_n = 0.f, dt_n = 0.f;
 #pragma unroll
   for (int u = 0; u < Q; ++u) q[u] = __ldcs(o + u);
   for (unsigned s = 0; s < cnt && !done; ++s) {
     if (s + 1 < cnt) {
 #pragma unroll
       for (int u = 0; u < Q; ++u) qn[u] = __ldcs(o + (size_t)(s + 1) * Q + u);
-      t_in_n = b.seg_tin[off + s + 1];
-      dt_n = b.seg_dt[off + s + 1];
+      const float2 tdn = b.seg_td[off + s + 1];
+      t_in_n = tdn.x;
+      dt_n = tdn.y;
     }
 #pragma unroll
     for (int u = 0; u < KK; ++u) {
@@ -85,8 +103,8 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, void* __rest
       s_begin = cnt;                       // nothing left for the general loop
     }
     for (unsigned s = s_begin; s < cnt && !done; ++s) {
-      const float t_in = b.seg_tin[off + s];
-      const float dt = b.seg_dt[off + s];
+      const float2 td = b.seg_td[off + s];
+      const float t_in = td.x, dt = td.y;
       const size_t o0 = (size_t)(off + s) * K;
       // the K samples of a segment are K consecutive float4 (uint2 on the tensor path): fetch them eight at a
       // time, back to back, so that every 128-byte line is requested once, whole, and not re-fetched after an
@@ -145,19 +163,7 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, void* __rest
       write_out = finished;
     }
     if (write_out) {
-      const size_t gr = (size_t)(f.out0 + (long long)r);
-      if (f.out_format == 0) {
-        float* o = reinterpret_cast<float*>(out_rgb) + gr * 3;
-        o[0] = C0; o[1] = C1; o[2] = C2;
-        reinterpret_cast<float*>(out_depth)[gr] = D;
-      } else {
-        // R360_OUT_RGB8_D16: colour rounded to the nearest of 256 levels, depth to binary16
-        uint8_t* o = reinterpret_cast<uint8_t*>(out_rgb) + gr * 3;
-        o[0] = (uint8_t)__float2int_rn(__saturatef(C0) * 255.0f);
-        o[1] = (uint8_t)__float2int_rn(__saturatef(C1) * 255.0f);
-        o[2] = (uint8_t)__float2int_rn(__saturatef(C2) * 255.0f);
-        reinterpret_cast<__half*>(out_depth)[gr] = __float2half_rn(D);
-      }
+      write_pixel(f, out_rgb, out_depth, (size_t)(f.out0 + (long long)r), C0, C1, C2, D);
     }
   }
   // samples_used statistic

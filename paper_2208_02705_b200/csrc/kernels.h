@@ -47,8 +47,7 @@ struct ChunkBuffers {
   unsigned long long* totals;  // [kTotN] device-side counters of the current ray chunk (indices below)
   unsigned long long* host_flags;  // mapped pinned host memory, [2]: k_scan posts {overflow flag, largest pass} of the
                                    // chunk here, so the host learns them without a copy in the stream
-  float* seg_tin;        // [G] ray-major
-  float* seg_dt;         // [G] ray-major
+  float2* seg_td;        // [G] ray-major (t_in, delta) of every segment: one 8-byte access per segment and lane
   SegRec* recs;          // [G * kRecWords] binned by subfield (common.cuh: SegRec)
   float4* out;           // [G*K] (sigma, r, g, b) per sample, ray-major; the tensor path stores a sample as four
                          // binary16 values (8 bytes, the same buffer read as uint2)

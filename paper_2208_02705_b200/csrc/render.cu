@@ -145,8 +145,7 @@ size_t out_bytes_per_segment(const r360_scene* sc) {
 
 // capacity of the segment buffers, in segments
 unsigned long long seg_capacity(const r360_scene* sc) {
-  size_t c = sc->seg_tin_cap;
-  if (sc->seg_dt_cap < c) c = sc->seg_dt_cap;
+  size_t c = sc->seg_td_cap;
   if (sc->recs_cap / kRecWords < c) c = sc->recs_cap / kRecWords;
   const size_t oc = sc->out_cap_bytes / out_bytes_per_segment(sc);
   if (oc < c) c = oc;
@@ -161,8 +160,7 @@ size_t expected_segments(const r360_scene* sc, size_t n_rays) {
 
 r360_status grow_segment_buffers(r360_scene* sc, size_t n_segs) {
   r360_status st;
-  if ((st = grow(sc->buf.seg_tin, sc->seg_tin_cap, n_segs)) != R360_OK) return st;
-  if ((st = grow(sc->buf.seg_dt, sc->seg_dt_cap, n_segs)) != R360_OK) return st;
+  if ((st = grow(sc->buf.seg_td, sc->seg_td_cap, n_segs)) != R360_OK) return st;
   if ((st = grow(sc->buf.recs, sc->recs_cap, n_segs * kRecWords)) != R360_OK) return st;
   unsigned char* o = reinterpret_cast<unsigned char*>(sc->buf.out);
   st = grow(o, sc->out_cap_bytes, n_segs * out_bytes_per_segment(sc));

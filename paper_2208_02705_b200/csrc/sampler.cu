@@ -384,8 +384,7 @@ k_emit(GridParams g, const uint16_t* __restrict__ grid, FrameParams f, ChunkBuff
       uint32_t pos = base + __popc(peers & lanemask_lt());
       b.recs[(size_t)pos * kRecWords] = make_uint4(r, __float_as_uint(t_in), __float_as_uint(dt), slot);
       b.recs[(size_t)pos * kRecWords + 1] = dir;
-      b.seg_tin[slot] = t_in;
-      b.seg_dt[slot] = dt;
+      b.seg_td[slot] = make_float2(t_in, dt);
       ++slot;
     }
   }

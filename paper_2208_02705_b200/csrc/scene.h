@@ -35,7 +35,7 @@ struct r360_scene {
   // chunk buffers and capacities
   r360::ChunkBuffers buf{};
   size_t ray_cnt_cap = 0, ray_off_cap = 0, blocks_cap = 0;
-  size_t seg_tin_cap = 0, seg_dt_cap = 0, recs_cap = 0, out_cap_bytes = 0, dirblk_cap = 0, hit_t_cap = 0, hit_lab_cap = 0, blk_list_cap = 0, blk_list_n_cap = 0;
+  size_t seg_td_cap = 0, recs_cap = 0, out_cap_bytes = 0, dirblk_cap = 0, hit_t_cap = 0, hit_lab_cap = 0, blk_list_cap = 0, blk_list_n_cap = 0;
   uint4* d_dirblk = nullptr;                // owned; buf.dirblk points here only while the tensor path is selected
   // pinned, mapped snapshots of the device counters, kMaxChunks x 2 x kTotN: [2c] = what k_scan posts for chunk c
   // (overflow flag, largest pass), [2c + 1] = the counters at the end of the chunk (statistics)
