@@ -104,7 +104,7 @@ constexpr int kBlkListCap = 256;
 
 void launch_count(const GridParams& g, const uint16_t* grid, const FrameParams& f, const ChunkBuffers& b,
                   int n_bins, cudaStream_t s);
-// seg_cap: capacity of the segment buffers (seg_tin, seg_dt, recs, out) in segments; later_wave_pass: a wavefront
+// seg_cap: capacity of the segment buffers (seg_td, recs, out) in segments; later_wave_pass: a wavefront
 // pass after the first (an empty one ends the chunk)
 void launch_scan(const ChunkBuffers& b, int n_blocks, int n_bins, int segs_per_tile, unsigned long long seg_cap,
                  int later_wave_pass, cudaStream_t s);

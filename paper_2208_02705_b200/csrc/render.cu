@@ -3,7 +3,7 @@
 // A call is cut into ray chunks (r360_set_chunk_rays); a chunk is 5 kernel launches (k_count, k_scan, k_emit,
 // k_mlp_*, k_composite), or one such group per pass with r360_set_wavefront.  The host never waits for the GPU
 // in the middle of a frame: the kernels behind k_scan take their counts from device memory (kernels.h: totals),
-// and the segment buffers (seg_tin, seg_dt, recs, out) are sized from a CAPACITY learnt from earlier frames
+// and the segment buffers (seg_td, recs, out) are sized from a CAPACITY learnt from earlier frames
 // (largest segments-per-ray ratio seen, plus a quarter).  If a chunk has more segments than the capacity, k_scan
 // raises kTotOverflow, the chunk's remaining kernels return at once, and the host -- which finds the flag in
 // mapped pinned memory at its next call on the scene (r360_settle: r360_wait, r360_get_stats, the next render
