@@ -292,6 +292,13 @@ r360_status r360_debug_samples(r360_scene* scene, const float pose[12], int32_t 
  * sm_mhz_out (may be NULL) receives the device's nominal SM clock. */
 r360_status r360_measure_fp32_fma(double* tflops_out, double* sm_mhz_out);
 
+/* The same plus steps a6-a9: the tiny MLPs are evaluated (in the scene's precision mode) and
+ *  field   DEVICE float[cap*4]  (sigma, r, g, b) of every sample, in the order of t / subfield
+ * is exported before any compositing -- the parity tap for the field (Eq.1, Table 4) sample by sample. */
+r360_status r360_debug_field(r360_scene* scene, const float pose[12], int32_t W, int32_t H,
+                             uint32_t* counts, uint32_t* offsets, float* t, int32_t* subfield, float* field,
+                             uint64_t cap, uint64_t* total);
+
 const char* r360_status_string(r360_status s);
 /* Text of the last CUDA error seen by this library on the calling thread ("" if none). */
 const char* r360_last_cuda_error(void);

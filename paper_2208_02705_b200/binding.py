@@ -115,6 +115,8 @@ def lib():
     L.r360_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.r360_debug_samples.restype = C.c_int
     L.r360_debug_samples.argtypes = [vp, f32p, i32, i32, vp, vp, vp, vp, C.c_uint64, C.POINTER(C.c_uint64)]
+    L.r360_debug_field.restype = C.c_int
+    L.r360_debug_field.argtypes = [vp, f32p, i32, i32, vp, vp, vp, vp, vp, C.c_uint64, C.POINTER(C.c_uint64)]
     L.r360_status_string.restype = C.c_char_p
     L.r360_status_string.argtypes = [C.c_int]
     L.r360_last_cuda_error.restype = C.c_char_p
@@ -429,6 +431,23 @@ class Scene:
         _check(st, "r360_debug_samples")
         n = int(total.value)
         return counts, offsets, t[:n], sid[:n]
+
+
+def _debug_field(self, pose, W, H):
+    """(counts, offsets, t, subfield, field[S, 4]) as torch CUDA tensors; steps a1-a9 (r360_debug_field)."""
+    import torch
+    counts, offsets, t, sid = self.debug_samples(pose, W, H)
+    n = int(t.numel())
+    field = torch.empty((max(n, 1), 4), dtype=torch.float32, device="cuda")
+    keep, p = _pose_ptr(pose, 1)
+    total = C.c_uint64(0)
+    _check(lib().r360_debug_field(self._h, p, W, H, counts.data_ptr(), offsets.data_ptr(), t.data_ptr(), sid.data_ptr(),
+                                  field.data_ptr(), max(n, 1), C.byref(total)), "r360_debug_field")
+    assert int(total.value) == n
+    return counts, offsets, t, sid, field[:n]
+
+
+Scene.debug_field = _debug_field
 
 
 def scene_from(sc, **override):

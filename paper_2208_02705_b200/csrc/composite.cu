@@ -172,6 +172,19 @@ k_composite(GridParams g, FrameParams f, ChunkBuffers b, float tau, void* __rest
   if ((threadIdx.x & 31) == 0 && used) atomicAdd(&b.totals[kTotUsed], (unsigned long long)used);
 }
 
+// debug tap: the per-sample MLP outputs (sigma, r, g, b), ray-major, as float4
+__global__ void k_export_field(ChunkBuffers b, size_t n_samples, int half_samples, float4* __restrict__ field) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n_samples) return;
+  field[i] = half_samples ? unpack_half4(reinterpret_cast<const uint2*>(b.out)[i]) : b.out[i];
+}
+
+void launch_export_field(const ChunkBuffers& b, size_t n_samples, bool half_samples, float* field, cudaStream_t s) {
+  if (!n_samples) return;
+  k_export_field<<<(unsigned)((n_samples + 255) / 256), 256, 0, s>>>(b, n_samples, half_samples ? 1 : 0,
+                                                                     reinterpret_cast<float4*>(field));
+}
+
 void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuffers& b, float tau,
                       void* out_rgb, void* out_depth, const PassParams& pp, bool half_samples, cudaStream_t s) {
   const dim3 grid((f.n_rays + 127) / 128), block(128);

@@ -129,6 +129,7 @@ void launch_composite(const GridParams& g, const FrameParams& f, const ChunkBuff
 // debug: expand binned records into ray-major per-sample t and subfield id
 void launch_export_samples(const GridParams& g, const ChunkBuffers& b, int n_bins, unsigned n_segs,
                            float* t, int32_t* subfield, cudaStream_t s);
+void launch_export_field(const ChunkBuffers& b, size_t n_samples, bool half_samples, float* field, cudaStream_t s);
 void launch_export_counts(const ChunkBuffers& b, unsigned n_rays, int K, uint32_t* counts, uint32_t* offsets,
                           cudaStream_t s);
 

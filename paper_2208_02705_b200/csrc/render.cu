@@ -170,10 +170,11 @@ r360_status grow_segment_buffers(r360_scene* sc, size_t n_segs) {
 
 // One chunk: steps a1-a10.  exact: wait for every k_scan and size the segment buffers from its count (first
 // chunk of a scene, retries, r360_debug_samples); otherwise nothing waits for the GPU.
-// sample_only: stop behind k_emit (r360_debug_samples); n_segs_out then receives the segment count.
+// sample_only: stop behind k_emit (r360_debug_samples), or behind the MLP kernel with stop_behind_mlp
+// (r360_debug_field); n_segs_out then receives the segment count.
 r360_status run_chunk(r360_scene* sc, int W, int H, const ChunkJob& job, unsigned chunk_idx, bool exact,
                       void* out_rgb, void* out_depth, unsigned& launches, bool sample_only = false,
-                      unsigned long long* n_segs_out = nullptr) {
+                      unsigned long long* n_segs_out = nullptr, bool stop_behind_mlp = false) {
   const int n = sc->desc.n_subfields;
   const FrameParams f = frame_params(sc, W, H, job);
   const size_t n_blocks = (f.n_rays + kSamplerThreads - 1) / kSamplerThreads;
@@ -267,7 +268,7 @@ r360_status run_chunk(r360_scene* sc, int W, int H, const ChunkJob& job, unsigne
     launches += 1;
     R360_CUDA(cudaGetLastError());
     if (timed) cudaEventRecord(ev->e[3], s);
-    if (sample_only) return R360_OK;
+    if (sample_only && !stop_behind_mlp) return R360_OK;
     cudaError_t e;
     if (sc->precision >= 1)
       e = launch_mlp_tc(sc->grid_p, f, sc->buf, sc->net, sc->precision == 2 ? sc->d_wpack_f16 : sc->d_wpack,
@@ -277,6 +278,7 @@ r360_status run_chunk(r360_scene* sc, int W, int H, const ChunkJob& job, unsigne
                           sc->n_sms, s);
     if (e != cudaSuccess) return r360_cuda_fail(e, "launch_mlp");
     launches += 1;
+    if (sample_only) return R360_OK;
     if (timed) cudaEventRecord(ev->e[4], s);
     launch_composite(sc->grid_p, f, sc->buf, sc->desc.t_threshold, out_rgb, out_depth, pp, sc->precision >= 1, s);
     launches += 1;
@@ -594,8 +596,26 @@ r360_status r360_get_stats(r360_scene* sc, r360_stats* out) {
   return R360_OK;
 }
 
+static r360_status debug_tap(r360_scene* sc, const float pose[12], int32_t W, int32_t H, uint32_t* counts,
+                             uint32_t* offsets, float* t, int32_t* subfield, float* field, bool with_field,
+                             uint64_t cap, uint64_t* total);
+
 r360_status r360_debug_samples(r360_scene* sc, const float pose[12], int32_t W, int32_t H, uint32_t* counts,
                                uint32_t* offsets, float* t, int32_t* subfield, uint64_t cap, uint64_t* total) {
+  return debug_tap(sc, pose, W, H, counts, offsets, t, subfield, nullptr, false, cap, total);
+}
+
+r360_status r360_debug_field(r360_scene* sc, const float pose[12], int32_t W, int32_t H, uint32_t* counts,
+                             uint32_t* offsets, float* t, int32_t* subfield, float* field, uint64_t cap,
+                             uint64_t* total) {
+  return debug_tap(sc, pose, W, H, counts, offsets, t, subfield, field, true, cap, total);
+}
+
+}  // extern "C"
+
+static r360_status debug_tap(r360_scene* sc, const float pose[12], int32_t W, int32_t H, uint32_t* counts,
+                             uint32_t* offsets, float* t, int32_t* subfield, float* field, bool with_field,
+                             uint64_t cap, uint64_t* total) {
   if (!sc || !pose || !counts || !offsets || !total || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
   if ((long long)W * H >= (1ll << 30)) return R360_ERR_INVALID_ARG;
   if (capturing(sc->stream)) return R360_ERR_INVALID_ARG;
@@ -606,7 +626,8 @@ r360_status r360_debug_samples(r360_scene* sc, const float pose[12], int32_t W, 
   const ChunkJob job{0, (unsigned)((long long)W * H), 0};
   unsigned long long n_segs = 0;
   unsigned launches = 0;
-  if ((st = run_chunk(sc, W, H, job, 0, /*exact=*/true, nullptr, nullptr, launches, /*sample_only=*/true, &n_segs)) != R360_OK)
+  if ((st = run_chunk(sc, W, H, job, 0, /*exact=*/true, nullptr, nullptr, launches, /*sample_only=*/true, &n_segs,
+                      /*stop_behind_mlp=*/with_field)) != R360_OK)
     return st;
   sc->chunks_last = 0;
   *total = n_segs * (uint64_t)sc->grid_p.K;
@@ -614,12 +635,11 @@ r360_status r360_debug_samples(r360_scene* sc, const float pose[12], int32_t W, 
   R360_CUDA(cudaGetLastError());
   if (*total > cap) { cudaStreamSynchronize(sc->stream); return R360_ERR_CAPACITY; }
   if (n_segs) {
-    if (!t || !subfield) return R360_ERR_INVALID_ARG;
+    if (!t || !subfield || (with_field && !field)) return R360_ERR_INVALID_ARG;
     launch_export_samples(sc->grid_p, sc->buf, sc->desc.n_subfields, (unsigned)n_segs, t, subfield, sc->stream);
+    if (with_field) launch_export_field(sc->buf, (size_t)n_segs * sc->grid_p.K, sc->precision >= 1, field, sc->stream);
     R360_CUDA(cudaGetLastError());
   }
   R360_CUDA(cudaStreamSynchronize(sc->stream));
   return R360_OK;
 }
-
-}  // extern "C"
