@@ -557,7 +557,8 @@ r360_status r360_set_stream(r360_scene* sc, void* stream) {
   if ((st = r360_settle(sc, true)) != R360_OK) return st;
   if ((cudaStream_t)stream != sc->stream) {
     // work of earlier calls on the old stream shares the scene's buffers with what follows on the new one
-    R360_CUDA(cudaStreamSynchronize(sc->stream));
+    // (the caller may already have destroyed the old stream: its work is complete then, the error is dropped)
+    if (cudaStreamSynchronize(sc->stream) != cudaSuccess) cudaGetLastError();
   }
   sc->stream = (cudaStream_t)stream;
   return R360_OK;
