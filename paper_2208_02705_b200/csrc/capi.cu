@@ -163,13 +163,14 @@ void r360_scene_destroy(r360_scene* sc) {
   cudaFree(sc->d_grid); cudaFree(sc->d_skip); cudaFree(sc->d_frames); cudaFree(sc->d_wt); cudaFree(sc->d_wpack); cudaFree(sc->d_wpack_f16);
   cudaFree(sc->d_tables); cudaFree(sc->d_poses);
   cudaFree(sc->buf.ray_cnt); cudaFree(sc->buf.ray_off); cudaFree(sc->buf.block_sum);
-  cudaFree(sc->buf.bin_cnt); cudaFree(sc->buf.bin_start); cudaFree(sc->buf.bin_cursor);
-  cudaFree(sc->buf.tile_start); cudaFree(sc->buf.totals);
+  cudaFree(sc->buf.totals);     // one allocation: totals | bin_cnt | bin_ovf
+  cudaFree(sc->buf.bin_start); cudaFree(sc->buf.bin_cursor);
+  cudaFree(sc->buf.tile_start);
   cudaDeviceSynchronize();   // (work of the last calls may still use the buffers)
   cudaFree(sc->buf.seg_td); cudaFree(sc->buf.recs); cudaFree(sc->buf.out);
   cudaFree(sc->d_dirblk);
   cudaFree(sc->buf.hit_t); cudaFree(sc->buf.hit_lab);
-  cudaFree(sc->buf.bin_ovf); cudaFree(sc->buf.blk_list); cudaFree(sc->buf.blk_list_n);
+  cudaFree(sc->buf.blk_list); cudaFree(sc->buf.blk_list_n);
   cudaFree(sc->d_pass_cnt); cudaFree(sc->buf.pass_off); cudaFree(sc->buf.st_c); cudaFree(sc->buf.st_T);
   for (int i = 0; i < 2; ++i) {
     cudaFree(sc->d_stage_rgb[i]); cudaFree(sc->d_stage_depth[i]);
@@ -317,12 +318,14 @@ r360_status r360_scene_create(const r360_scene_desc* desc, const uint8_t* occupa
       R360_CUDA(cudaMemcpy(sc->d_wpack_f16, wpack16.data(), wpack16.size(), cudaMemcpyHostToDevice));
     }
   }
-  R360_CUDA(cudaMalloc(&sc->buf.bin_cnt, (size_t)n * 4));
-  R360_CUDA(cudaMalloc(&sc->buf.bin_ovf, (size_t)n * 4));
+  // the counters that are cleared at the start of a chunk sit in ONE allocation, cleared by one memset:
+  // totals[kTotN] | bin_cnt[n] | bin_ovf[n]
+  R360_CUDA(cudaMalloc(&sc->buf.totals, kTotN * sizeof(unsigned long long) + (size_t)n * 8));
+  sc->buf.bin_cnt = reinterpret_cast<uint32_t*>(sc->buf.totals + kTotN);
+  sc->buf.bin_ovf = sc->buf.bin_cnt + n;
   R360_CUDA(cudaMalloc(&sc->buf.bin_start, (size_t)(n + 1) * 4));
   R360_CUDA(cudaMalloc(&sc->buf.bin_cursor, (size_t)n * 4));
   R360_CUDA(cudaMalloc(&sc->buf.tile_start, (size_t)(n + 1) * 4));
-  R360_CUDA(cudaMalloc(&sc->buf.totals, kTotN * sizeof(unsigned long long)));
   {
     const size_t bytes = (size_t)r360_scene::kMaxChunks * 2 * kTotN * sizeof(unsigned long long);
     R360_CUDA(cudaHostAlloc(&sc->h_snap, bytes, cudaHostAllocMapped));

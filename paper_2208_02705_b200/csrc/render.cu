@@ -216,7 +216,6 @@ r360_status run_chunk(r360_scene* sc, int W, int H, const ChunkJob& job, unsigne
   // pinned slots of this chunk: [2c] = {overflow flag, largest pass} posted by k_scan, [2c + 1] = the counters
   unsigned long long* snap_tot = sc->h_snap + ((size_t)chunk_idx * 2 + 1) * kTotN;
   sc->buf.host_flags = sc->d_snap + (size_t)chunk_idx * 2 * kTotN;
-  R360_CUDA(cudaMemsetAsync(sc->buf.totals, 0, kTotN * sizeof(unsigned long long), s));
   // single pass over all hits, or the wavefront passes (kernels.h: PassParams)
   static const uint32_t kPassEnd[5] = {2, 6, 16, (uint32_t)kHitCap, 0xFFFFFFFFu};
   const int n_pass = wave ? 5 : 1;
@@ -230,8 +229,10 @@ r360_status run_chunk(r360_scene* sc, int W, int H, const ChunkJob& job, unsigne
       pp.h1 = kPassEnd[p];
     }
     const bool timed = p == 0 && !cap;                         // stage times: first pass only
-    R360_CUDA(cudaMemsetAsync(sc->buf.bin_cnt, 0, (size_t)n * 4, s));
-    R360_CUDA(cudaMemsetAsync(sc->buf.bin_ovf, 0, (size_t)n * 4, s));
+    // totals | bin_cnt | bin_ovf are one allocation (capi.cu): the chunk's first pass clears all of it with one
+    // memset, a later wavefront pass only the two histograms
+    if (p == 0) R360_CUDA(cudaMemsetAsync(sc->buf.totals, 0, kTotN * sizeof(unsigned long long) + (size_t)n * 8, s));
+    else R360_CUDA(cudaMemsetAsync(sc->buf.bin_cnt, 0, (size_t)n * 8, s));
     if (timed) cudaEventRecord(ev->e[0], s);
     if (!wave || pp.first) {
       launch_count(sc->grid_p, sc->d_grid, f, sc->buf, n, s);
