@@ -127,7 +127,8 @@ __device__ __forceinline__ float plane(const GridParams& g, int a, int k) {
 // cube [idx, idx + (D-1) step] at once: the exit distance `to` is the smallest far-plane distance of the
 // CUBE, the axis of the minimum steps to the voxel behind that plane, and on the other two axes the new
 // index is the first one (along the ray) whose far plane lies beyond `to` -- found from a position guess
-// and then verified against the planes themselves, so no rounding of the guess can change the result.
+// that is checked against the planes themselves (a too large guess is walked back here, a too small one
+// corrects itself in the next iteration, see advance()), so no rounding of the guess can change the result.
 // The entry distance of the next voxel is max(t0, to, its near planes), which is exactly the
 // oracle's max(t0, tn_x, tn_y, tn_z); for a plain one-voxel step this reduces to max(ti, to).
 struct Walker {
@@ -231,13 +232,14 @@ struct Walker {
             const int lo = off[a] ? idx[a] : max(idx[a] - r, 0), hi = off[a] ? min(idx[a] + r, g.dims[a] - 1) : idx[a];
             const int first = idx[a];
             const float p = __fmaf_rn(to, d[a], o[a]);
-            int gi = __float2int_rd((p - g.box_min[a]) * g.inv_vs[a]);     // guess, verified below
+            int gi = __float2int_rd((p - g.box_min[a]) * g.inv_vs[a]);     // guess; a too large one is corrected below
             gi = min(max(gi, lo), hi);
-            // forward: the far plane of gi must lie beyond `to`
-            while (!(t_at(g, a, gi + off[a]) > to)) {
-              gi += step[a];
-              if ((unsigned)gi >= (unsigned)g.dims[a]) { alive = false; break; }
-            }
+            // (A guess that is too SMALL needs no check here.  The voxel it names is then left at or before `to`:
+            // its far plane on this axis is <= to <= the entry distance set below, so the next iteration finds
+            // t_in >= t_out for it -- not crossed, nothing emitted, whatever it holds -- and steps across that
+            // very plane with the entry distance unchanged; if it is empty with a skip cube, the cube holds the
+            // ray's true voxel and is empty, so leaving it at once is as valid.  One plane distance per axis less
+            // in every cube exit, one cheap extra iteration when the guess was off.)
             // backward: no earlier index of the cube may qualify; tn = near plane of gi
             float tn = t_at(g, a, gi - step[a] + off[a]);
             while (gi != first && tn > to) {
