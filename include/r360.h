@@ -218,6 +218,37 @@ r360_status r360_fusion_fuse_device(r360_fusion* fusion, const float pose[12], i
 r360_status r360_fusion_read(r360_fusion* fusion, float* logodds_out, uint8_t* occupancy_out);
 void r360_fusion_destroy(r360_fusion* fusion);
 
+/* One observation of Eq. 6 WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc:
+ * a program whose own arena or caching allocator already holds the whole GPU (a library allocation would fail or
+ * fragment it), a frame loop that cannot afford the device-wide stall cudaMalloc / cudaFree may cause, or code that
+ * runs at a moment when its process forbids allocation (e.g. another thread is recording a CUDA graph in the global
+ * capture mode).  r360_fusion_create / r360_fusion_fuse* allocate (grid-sized scratch at create, tables and staging
+ * whenever the image size changes); this call uses neither cudaMalloc nor cudaFree nor any allocating library
+ * routine.  Same arithmetic and same kernels as r360_fusion_fuse_device: the grid is equal bit for bit.
+ *  dims, box_min, box_max  HOST, as in r360_fusion_create
+ *  logodds      DEVICE float[N], N = Nx*Ny*Nz, read and written in place (the caller's grid; this call keeps no state)
+ *  pose         HOST float[12] as in r360_render; read before the call returns
+ *  depth        DEVICE float[H*W];  uncertainty  DEVICE float[H*W] or NULL
+ *  cuda_stream  cudaStream_t as void* (NULL = the default stream); all work is enqueued on it, the call does not wait
+ * Scratch: the per-voxel flags and minimum uncertainty (8 bytes per voxel), the pixel-angle tables and the pose live
+ * in one static device array of 64 MiB + 48 KiB inside libr360.so.  Every GPU that loads the library holds it until
+ * the process exits, and it bounds the problem: N <= R360_STATIC_MAX_VOXELS, W <= R360_STATIC_MAX_W,
+ * H <= R360_STATIC_MAX_H; anything larger returns R360_ERR_CAPACITY before any GPU work (r360_last_cuda_error() then
+ * names the limits) -- use the r360_fusion handle for such grids.
+ * The FIRST call on each device looks up the array's device address (once, with that device current) and may make
+ * the CUDA runtime load the library's kernels: make that first call during set-up, before any stream capture.
+ * Every call on a device shares the one array and leaves its last contents there; a call resets the part it uses
+ * before its kernels run.  Calls whose GPU work can overlap (two streams, two host threads with their own streams)
+ * race on it: keep all calls of a device on one stream, or order them with events.
+ * Errors: INVALID_ARG (NULL pointers, dims < 1, box_max <= box_min, W or H < 1, non-finite pose, device ordinal
+ * >= 64), CAPACITY (see above), CUDA. */
+#define R360_STATIC_MAX_VOXELS (8u << 20) /* 8 Mi voxels: covers 256 x 256 x 96 (BASELINE configs 1-3, 5)     */
+#define R360_STATIC_MAX_W 4096
+#define R360_STATIC_MAX_H 2048
+r360_status r360_fusion_fuse_static(const int32_t dims[3], const float box_min[3], const float box_max[3],
+                                    float* logodds, const float pose[12], int32_t W, int32_t H, const float* depth,
+                                    const float* uncertainty, void* cuda_stream);
+
 /* Camera of the following render / debug calls.  model 0 (default) = the equirectangular panorama of
  * Eq.2-3; model 1 = pinhole view for roaming (the paper's perspective display,
  * PAPER.md:206, :200, gives no model; reading P): pixel centre (i+0.5, j+0.5) ->

@@ -5,9 +5,9 @@ Thin ctypes binding over the C ABI in include/r360.h (libr360.so, hand-written C
 sm_100a).  Argument marshalling only: every step of the path runs in the CUDA kernels.
 There is no CPU fallback; loading fails loudly if the library is missing.
 """
-from .binding import (Fusion, R360Error, Scene, Stats, assign_subfields, floorplan, occupancy_fuse, lib,
+from .binding import (Fusion, fusion_fuse_static, STATIC_MAX_VOXELS, STATIC_MAX_W, STATIC_MAX_H, R360Error, Scene, Stats, assign_subfields, floorplan, occupancy_fuse, lib,
                       lib_path, measure_fp32_fma, params_per_subfield, scene_from,
                       version, STATUS)
 
-__all__ = ["Fusion", "R360Error", "Scene", "Stats", "assign_subfields", "floorplan", "occupancy_fuse", "lib", "lib_path", "measure_fp32_fma", "params_per_subfield", "scene_from", "version",
+__all__ = ["Fusion", "fusion_fuse_static", "STATIC_MAX_VOXELS", "STATIC_MAX_W", "STATIC_MAX_H", "R360Error", "Scene", "Stats", "assign_subfields", "floorplan", "occupancy_fuse", "lib", "lib_path", "measure_fp32_fma", "params_per_subfield", "scene_from", "version",
            "STATUS"]

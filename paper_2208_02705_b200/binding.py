@@ -241,6 +241,41 @@ class Fusion:
             pass
 
 
+STATIC_MAX_VOXELS, STATIC_MAX_W, STATIC_MAX_H = 8 << 20, 4096, 2048   # R360_STATIC_MAX_* of include/r360.h
+
+
+def fusion_fuse_static(logodds, dims, box_min, box_max, pose, W, H, depth, uncertainty=None, stream=None):
+    """One observation of Eq. 6 fused in place into `logodds` without any device allocation
+    (r360_fusion_fuse_static).  For callers that cannot call cudaMalloc: a process whose own pool already holds the
+    whole GPU, a frame loop that cannot take an allocation's device-wide stall, code running while allocation is
+    forbidden.  The scratch is a static array inside libr360.so, which limits the problem to STATIC_MAX_VOXELS
+    voxels and a STATIC_MAX_W x STATIC_MAX_H image.
+
+    logodds: torch CUDA float32 tensor [Nx*Ny*Nz], updated in place; depth / uncertainty: torch CUDA float32 tensors
+    of W*H elements; stream: a torch.cuda.Stream, a raw cudaStream_t as int, or None for the default stream.
+    Asynchronous.  All calls on one device share the scratch: keep them on one stream (overlapping calls race).
+    Make the first call on a device during set-up (it resolves the scratch's device address)."""
+    fn = lib().r360_fusion_fuse_static
+    if fn.argtypes is None:
+        f32p = C.POINTER(C.c_float)
+        fn.restype = C.c_int
+        fn.argtypes = [C.POINTER(C.c_int32), f32p, f32p, C.c_void_p, f32p, C.c_int32, C.c_int32, C.c_void_p,
+                       C.c_void_p, C.c_void_p]
+    d = (C.c_int32 * 3)(*[int(v) for v in dims])
+    lo = (C.c_float * 3)(*[float(v) for v in box_min])
+    hi = (C.c_float * 3)(*[float(v) for v in box_max])
+    N = d[0] * d[1] * d[2]
+    for t, n in ((logodds, N), (depth, W * H)) + (() if uncertainty is None else ((uncertainty, W * H),)):
+        assert t.is_cuda and t.is_contiguous() and t.numel() == n and t.element_size() == 4
+    p = np.ascontiguousarray(pose, np.float32).reshape(12)
+    s = None if stream is None else int(getattr(stream, "cuda_stream", stream))
+    st = fn(d, lo, hi, logodds.data_ptr(), p.ctypes.data_as(C.POINTER(C.c_float)), int(W), int(H), depth.data_ptr(),
+            None if uncertainty is None else uncertainty.data_ptr(), s)
+    if st == 6:
+        raise R360Error(st, "r360_fusion_fuse_static", lib().r360_last_cuda_error().decode())
+    _check(st, "r360_fusion_fuse_static")
+
+
 def floorplan(occupancy, dims, occ_threshold, seed_xy, upper=None, lower=None):
     """Floorplan from the occupancy map on the GPU (r360_floorplan): uint8 [Ny][Nx], bit 0 interior, bit 1 inner
     boundary, bit 2 obstacle."""

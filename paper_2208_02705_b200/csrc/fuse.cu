@@ -12,6 +12,8 @@
 //   k_update : one thread per voxel applies Eq. 6 once and clears the flags
 // The result does not depend on the order of the rays (flags and a minimum), so it is reproducible bit for bit.
 #include <cmath>
+#include <cstdio>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -278,3 +280,127 @@ r360_status r360_occupancy_fuse(const int32_t dims[3], const float box_min[3], c
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------
+// r360_fusion_fuse_static: one observation of Eq. 6 for callers that must not allocate device memory.
+//
+// Who that is: a host program that has handed the whole GPU to its own arena or caching allocator (a later
+// cudaMalloc from a library would fail or fragment it), a frame loop that cannot take the device-wide stall a
+// cudaMalloc / cudaFree may cause, and code that runs while allocation is forbidden in its process (for example
+// while some other thread records a CUDA graph in the global capture mode).  The r360_fusion handle allocates at
+// create time and again whenever the image size changes; this entry point never allocates: the per-voxel flags, the
+// per-voxel minimum uncertainty, the pixel-angle tables and the pose live in ONE file-scope device array of fixed
+// size.  The price is a fixed limit (R360_STATIC_MAX_VOXELS, R360_STATIC_MAX_W, R360_STATIC_MAX_H) and
+// kStaticBytes (64 MiB + 48 KiB) of device memory on every GPU that loads libr360.so, from load until exit.
+//
+// In host code the name g_fuse_scratch is only a handle for the runtime, not a device address: the address comes
+// from cudaGetSymbolAddress, asked once per device with that device current (static_scratch below).
+namespace {
+
+constexpr size_t kStaticMaxVoxels = R360_STATIC_MAX_VOXELS;
+constexpr int kStaticMaxW = R360_STATIC_MAX_W, kStaticMaxH = R360_STATIC_MAX_H;
+constexpr size_t kStaticTabFloats = 2 * (size_t)kStaticMaxW + 2 * (size_t)kStaticMaxH;
+// layout: flags uint32[kStaticMaxVoxels] | umin uint32[kStaticMaxVoxels] | tables float[kStaticTabFloats] | pose float[16]
+constexpr size_t kStaticOffUmin = kStaticMaxVoxels * sizeof(uint32_t);
+constexpr size_t kStaticOffTab = 2 * kStaticOffUmin;
+constexpr size_t kStaticOffPose = kStaticOffTab + kStaticTabFloats * sizeof(float);
+constexpr size_t kStaticBytes = kStaticOffPose + 16 * sizeof(float);
+static_assert(kStaticOffTab % 256 == 0 && kStaticOffPose % 256 == 0, "sub-buffers keep the array's alignment");
+
+static __device__ __align__(256) unsigned char g_fuse_scratch[kStaticBytes];
+
+constexpr int kStaticMaxDevices = 64;
+struct StaticDev {
+  unsigned char* base = nullptr;    // device address of g_fuse_scratch on this device
+  int tab_W = 0, tab_H = 0;         // image size the tables in the scratch were built for
+};
+StaticDev g_static_dev[kStaticMaxDevices];
+std::mutex g_static_mu;
+
+// set-up, once per device, with that device current
+r360_status static_scratch(StaticDev** out) {
+  int dev = -1;
+  R360_CUDA(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kStaticMaxDevices) return R360_ERR_INVALID_ARG;
+  StaticDev& sd = g_static_dev[dev];
+  if (!sd.base) {
+    void* p = nullptr;
+    R360_CUDA(cudaGetSymbolAddress(&p, g_fuse_scratch));
+    if (!p) return R360_ERR_CUDA;
+    sd.base = static_cast<unsigned char*>(p);
+  }
+  *out = &sd;
+  return R360_OK;
+}
+
+}  // namespace
+
+extern "C" r360_status r360_fusion_fuse_static(const int32_t dims[3], const float box_min[3], const float box_max[3],
+                                               float* logodds, const float pose[12], int32_t W, int32_t H,
+                                               const float* depth, const float* uncertainty, void* cuda_stream) {
+  if (!dims || !box_min || !box_max || !logodds || !pose || !depth || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
+  r360::GridParams g{};
+  for (int a = 0; a < 3; ++a) {
+    if (dims[a] < 1 || !(box_max[a] > box_min[a])) return R360_ERR_INVALID_ARG;
+    g.dims[a] = dims[a];
+    g.box_min[a] = box_min[a];
+    volatile float ext = box_max[a] - box_min[a];               // voxel size exactly as r360_fusion_create computes it
+    g.vs[a] = ext / (float)dims[a];
+    g.inv_vs[a] = 1.0f / g.vs[a];
+  }
+  for (int i = 0; i < 12; ++i)
+    if (!std::isfinite(pose[i])) return R360_ERR_INVALID_ARG;
+  const unsigned long long N64 = (unsigned long long)dims[0] * (unsigned long long)dims[1] * (unsigned long long)dims[2];
+  if (N64 > kStaticMaxVoxels || W > kStaticMaxW || H > kStaticMaxH) {
+    // the text r360_last_cuda_error() returns names the limit that was hit
+    char msg[200];
+    snprintf(msg, sizeof(msg), "r360_fusion_fuse_static: %llu voxels, %d x %d image exceed the static scratch "
+             "(at most %zu voxels, %d x %d)", N64, W, H, kStaticMaxVoxels, kStaticMaxW, kStaticMaxH);
+    r360_cuda_fail(cudaErrorInvalidValue, msg);
+    return R360_ERR_CAPACITY;
+  }
+  const size_t N = (size_t)N64, R = (size_t)W * H;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  StaticDev* sd = nullptr;
+  const r360_status st = static_scratch(&sd);
+  if (st != R360_OK) return st;
+  uint32_t* flags = reinterpret_cast<uint32_t*>(sd->base);
+  uint32_t* umin = reinterpret_cast<uint32_t*>(sd->base + kStaticOffUmin);
+  float* d_tab = reinterpret_cast<float*>(sd->base + kStaticOffTab);
+  float* d_pose = reinterpret_cast<float*>(sd->base + kStaticOffPose);
+  if (sd->tab_W != W || sd->tab_H != H) {
+    // reading B2: trig of the pixel-centre angles in binary64, rounded once (the same expressions as above).  The
+    // source is pageable stack memory: cudaMemcpyAsync has staged it when it returns.
+    const double kPi = 3.14159265358979323846;
+    float tab[kStaticTabFloats];
+    for (int i = 0; i < W; ++i) {
+      const double phi = (((double)i + 0.5) - (double)W / 2.0) * (2.0 * kPi / (double)W);
+      tab[i] = (float)std::sin(phi);
+      tab[(size_t)W + i] = (float)std::cos(phi);
+    }
+    for (int j = 0; j < H; ++j) {
+      const double theta = -((((double)j + 0.5) - (double)H / 2.0) * (kPi / (double)H));
+      tab[(size_t)2 * W + j] = (float)std::sin(theta);
+      tab[(size_t)2 * W + H + j] = (float)std::cos(theta);
+    }
+    sd->tab_W = sd->tab_H = 0;
+    R360_CUDA(cudaMemcpyAsync(d_tab, tab, ((size_t)2 * W + 2 * H) * sizeof(float), cudaMemcpyHostToDevice, stream));
+    sd->tab_W = W;
+    sd->tab_H = H;
+  }
+  R360_CUDA(cudaMemcpyAsync(d_pose, pose, 12 * sizeof(float), cudaMemcpyHostToDevice, stream));
+  // the array keeps what the last call (any grid size, possibly a failed one) left in it: the part this call uses
+  // starts from "no flag, uncertainty 1.0" again
+  R360_CUDA(cudaMemsetAsync(flags, 0, N * sizeof(uint32_t), stream));
+  k_fill_u32<<<(unsigned)((N + 255) / 256), 256, 0, stream>>>(umin, N, 0x3F800000u);
+  r360::FrameParams f{};
+  f.W = W; f.H = H; f.ray0 = 0; f.pose0 = 0; f.pix0 = 0; f.n_rays = (unsigned)R; f.camera = 0;
+  f.poses = d_pose;
+  f.sin_phi = d_tab; f.cos_phi = d_tab + W;
+  f.sin_theta = d_tab + 2 * (size_t)W; f.cos_theta = d_tab + 2 * (size_t)W + H;
+  k_mark<<<(unsigned)((R + 255) / 256), 256, 0, stream>>>(g, f, depth, uncertainty, flags, umin);
+  k_update<<<(unsigned)((N + 255) / 256), 256, 0, stream>>>(N, (float)std::log(0.4 / 0.6), logodds, flags, umin);
+  R360_CUDA(cudaGetLastError());
+  return R360_OK;
+}
