@@ -157,7 +157,15 @@ r360_status r360_reserve(r360_scene* scene, uint64_t max_rays_per_chunk, double 
  * pinned buffer of the scene at every replay: r360_set_graph_poses replaces them between replays (host memcpy,
  * no CUDA call).  A replay cannot re-render a chunk that outgrew the buffers: r360_graph_status synchronises the
  * stream and returns R360_ERR_CAPACITY if the last replay hit that case (its outputs are then incomplete; call
- * r360_reserve with a larger ratio and capture again), R360_OK otherwise. */
+ * r360_reserve with a larger ratio and capture again), R360_OK otherwise.
+ * A graph holds the ADDRESSES and capacities of the scene's buffers as they were at capture.  Any later call outside
+ * a capture that frees or reallocates one of them makes the graph STALE, and a replay would touch freed memory: a
+ * larger frame or chunk, another image size or camera (new pixel tables), more poses per batch, a chunk that had to be
+ * re-rendered with larger buffers, r360_reserve, a switch to the tensor path or to wavefront passes for the first
+ * time.  The scene counts these events: for a stale graph r360_graph_status and r360_set_graph_poses return
+ * R360_ERR_CAPACITY -- check one of them before every replay that follows other calls on the scene, and capture again.
+ * Call r360_wait before cudaStreamBeginCapture: a captured render call returns R360_ERR_INVALID_ARG while chunks of the
+ * previous frame are still unverified (inside a capture they could not be re-rendered and would be lost). */
 r360_status r360_set_graph_poses(r360_scene* scene, const float* poses, int32_t B);
 r360_status r360_graph_status(r360_scene* scene);
 
@@ -207,7 +215,13 @@ r360_status r360_occupancy_fuse(const int32_t dims[3], const float box_min[3], c
  * number of observations (r360_fusion_fuse: HOST depth / uncertainty images; r360_fusion_fuse_device: DEVICE images,
  * e.g. the depth output of r360_render), read back when needed (logodds_out: HOST float[N] or NULL; occupancy_out:
  * HOST uint8[N] or NULL, 255 where logit > ln(0.97/0.03), else 0 -- the occupancy input of r360_scene_create with
- * occ_threshold 128).  Work runs on the default stream of the current device; r360_fusion_read synchronises. */
+ * occ_threshold 128).  Work runs on the default (legacy) stream of the current device; r360_fusion_read synchronises.
+ * Feeding r360_fusion_fuse_device from r360_render: the render calls are asynchronous and run on the scene's stream,
+ * so (1) call r360_wait(scene) first -- a chunk that outgrew its buffers is only complete after that -- and (2) if the
+ * scene's stream does not synchronise with the legacy default stream (a cudaStreamNonBlocking stream, or a process
+ * built with per-thread default streams), order the two yourself: cudaStreamSynchronize(scene stream), or an event
+ * recorded there and waited for on stream 0, before r360_fusion_fuse_device.  With the scene on stream 0 (the
+ * default) or on an ordinary blocking stream, r360_wait alone is enough. */
 typedef struct r360_fusion r360_fusion;
 r360_status r360_fusion_create(const int32_t dims[3], const float box_min[3], const float box_max[3],
                                const float* logodds_init, r360_fusion** out);

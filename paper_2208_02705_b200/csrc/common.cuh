@@ -26,7 +26,8 @@ struct GridParams {
   float box_min[3];
   float vs[3];           // voxel size per axis: (box_max - box_min) / dims, binary32 (reading C)
   float inv_vs[3];       // 1 / vs: only for index GUESSES that are then verified against the planes
-  const uint8_t* skip;   // device, [N][8]: octant skip distances of the empty voxels (above); null = no skipping
+  const uint8_t* skip;   // device, [N][8]: octant skip distances of the empty voxels (above); REQUIRED by the Walker (never
+                         // null: r360_scene_create always builds it; the fusion walk in fuse.cu does not use the Walker)
   int K;                 // samples per occupied voxel crossed (reading D)
   float Kf;
   float Kinv;            // 1 / K when K is a power of two (x * Kinv is then x / K bit for bit), else 0

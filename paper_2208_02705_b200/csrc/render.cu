@@ -25,10 +25,14 @@ constexpr double kPi = 3.14159265358979323846;
 // Inside a stream capture nothing may be allocated (g_no_alloc): a buffer that is too small is R360_ERR_CAPACITY.
 thread_local bool g_no_alloc = false;
 
+// Every free or reallocation of a buffer that a captured CUDA graph may have baked in (chunk buffers, tables,
+// poses) bumps the scene's buffer generation: a graph captured at an older generation must not be replayed
+// (r360_graph_status, r360_set_graph_poses).
 template <typename T>
-r360_status grow(T*& p, size_t& cap, size_t need) {
+r360_status grow(r360_scene* sc, T*& p, size_t& cap, size_t need) {
   if (need <= cap && p) return R360_OK;
   if (g_no_alloc) return R360_ERR_CAPACITY;
+  sc->buf_gen += 1;
   if (p) { cudaFree(p); p = nullptr; }           // (waits for the work that still uses it)
   const size_t want = need + 64;
   cudaError_t e = cudaMalloc(&p, want * sizeof(T));
@@ -67,6 +71,7 @@ r360_status ensure_tables(r360_scene* sc, int W, int H) {
     t[(size_t)2 * W + H + j] = (float)std::cos(theta);
   }
   // earlier frames may still be reading the old tables: cudaFree waits for the device
+  sc->buf_gen += 1;
   if (sc->d_tables) { cudaFree(sc->d_tables); sc->d_tables = nullptr; }
   R360_CUDA(cudaMalloc(&sc->d_tables, t.size() * sizeof(float)));
   // copy from a stack-owned vector; ordered before later work on sc->stream by a sync
@@ -85,6 +90,7 @@ r360_status upload_poses(r360_scene* sc, const float* poses, int B) {
   const bool cap = capturing(sc->stream);
   if (B > sc->poses_cap) {
     if (cap) return R360_ERR_CAPACITY;
+    sc->buf_gen += 1;
     if (sc->d_poses) { cudaFree(sc->d_poses); sc->d_poses = nullptr; }
     if (sc->h_poses) { cudaFreeHost(sc->h_poses); sc->h_poses = nullptr; }
     sc->poses_cap = 0;
@@ -160,10 +166,10 @@ size_t expected_segments(const r360_scene* sc, size_t n_rays) {
 
 r360_status grow_segment_buffers(r360_scene* sc, size_t n_segs) {
   r360_status st;
-  if ((st = grow(sc->buf.seg_td, sc->seg_td_cap, n_segs)) != R360_OK) return st;
-  if ((st = grow(sc->buf.recs, sc->recs_cap, n_segs * kRecWords)) != R360_OK) return st;
+  if ((st = grow(sc, sc->buf.seg_td, sc->seg_td_cap, n_segs)) != R360_OK) return st;
+  if ((st = grow(sc, sc->buf.recs, sc->recs_cap, n_segs * kRecWords)) != R360_OK) return st;
   unsigned char* o = reinterpret_cast<unsigned char*>(sc->buf.out);
-  st = grow(o, sc->out_cap_bytes, n_segs * out_bytes_per_segment(sc));
+  st = grow(sc, o, sc->out_cap_bytes, n_segs * out_bytes_per_segment(sc));
   sc->buf.out = reinterpret_cast<float4*>(o);
   return st;
 }
@@ -186,27 +192,27 @@ r360_status run_chunk(r360_scene* sc, int W, int H, const ChunkJob& job, unsigne
     explicit NoAlloc(bool on) { g_no_alloc = on; }
     ~NoAlloc() { g_no_alloc = false; }
   } no_alloc(cap);
-  if ((st = grow(sc->buf.ray_cnt, sc->ray_cnt_cap, f.n_rays)) != R360_OK) return st;
-  if ((st = grow(sc->buf.ray_off, sc->ray_off_cap, f.n_rays)) != R360_OK) return st;
-  if ((st = grow(sc->buf.block_sum, sc->blocks_cap, n_blocks)) != R360_OK) return st;
-  if ((st = grow(sc->buf.hit_t, sc->hit_t_cap, (size_t)f.n_rays * kHitCap)) != R360_OK) return st;
-  if ((st = grow(sc->buf.hit_lab, sc->hit_lab_cap, (size_t)f.n_rays * kHitCap)) != R360_OK) return st;
+  if ((st = grow(sc, sc->buf.ray_cnt, sc->ray_cnt_cap, f.n_rays)) != R360_OK) return st;
+  if ((st = grow(sc, sc->buf.ray_off, sc->ray_off_cap, f.n_rays)) != R360_OK) return st;
+  if ((st = grow(sc, sc->buf.block_sum, sc->blocks_cap, n_blocks)) != R360_OK) return st;
+  if ((st = grow(sc, sc->buf.hit_t, sc->hit_t_cap, (size_t)f.n_rays * kHitCap)) != R360_OK) return st;
+  if ((st = grow(sc, sc->buf.hit_lab, sc->hit_lab_cap, (size_t)f.n_rays * kHitCap)) != R360_OK) return st;
   if (sc->precision >= 1) {            // tensor path: per-ray records (direction + packed F(d))
-    if ((st = grow(sc->d_dirblk, sc->dirblk_cap, (size_t)f.n_rays * 4)) != R360_OK) return st;
+    if ((st = grow(sc, sc->d_dirblk, sc->dirblk_cap, (size_t)f.n_rays * 4)) != R360_OK) return st;
     sc->buf.dirblk = sc->d_dirblk;
     sc->buf.dir_f16 = sc->precision == 2;
   } else {
     sc->buf.dirblk = nullptr;
   }
-  if ((st = grow(sc->buf.blk_list, sc->blk_list_cap, n_blocks * kBlkListCap)) != R360_OK) return st;
-  if ((st = grow(sc->buf.blk_list_n, sc->blk_list_n_cap, n_blocks)) != R360_OK) return st;
+  if ((st = grow(sc, sc->buf.blk_list, sc->blk_list_cap, n_blocks * kBlkListCap)) != R360_OK) return st;
+  if ((st = grow(sc, sc->buf.blk_list_n, sc->blk_list_n_cap, n_blocks)) != R360_OK) return st;
   sc->buf.pass_cnt = nullptr;
   const bool wave = sc->wave_now && !sample_only;
   if (wave) {
-    if ((st = grow(sc->d_pass_cnt, sc->pass_cnt_cap, f.n_rays)) != R360_OK) return st;
-    if ((st = grow(sc->buf.pass_off, sc->pass_off_cap, f.n_rays)) != R360_OK) return st;
-    if ((st = grow(sc->buf.st_c, sc->st_c_cap, f.n_rays)) != R360_OK) return st;
-    if ((st = grow(sc->buf.st_T, sc->st_T_cap, f.n_rays)) != R360_OK) return st;
+    if ((st = grow(sc, sc->d_pass_cnt, sc->pass_cnt_cap, f.n_rays)) != R360_OK) return st;
+    if ((st = grow(sc, sc->buf.pass_off, sc->pass_off_cap, f.n_rays)) != R360_OK) return st;
+    if ((st = grow(sc, sc->buf.st_c, sc->st_c_cap, f.n_rays)) != R360_OK) return st;
+    if ((st = grow(sc, sc->buf.st_T, sc->st_T_cap, f.n_rays)) != R360_OK) return st;
     sc->buf.pass_cnt = sc->d_pass_cnt;
   }
   if (!exact && (st = grow_segment_buffers(sc, expected_segments(sc, f.n_rays))) != R360_OK) return st;
@@ -347,6 +353,9 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
   r360_status st;
   const bool cap = capturing(sc->stream);
   if (!cap && (st = r360_settle(sc, true)) != R360_OK) return st;
+  // inside a capture nothing can be re-rendered: chunks of the previous frame that nobody has verified yet (no
+  // r360_wait before cudaStreamBeginCapture) would stay incomplete for good once this call drops them
+  if (cap && sc->pending.next < sc->pending.chunks.size()) return R360_ERR_INVALID_ARG;
   if ((st = ensure_tables(sc, W, H)) != R360_OK) return st;
   if ((st = upload_poses(sc, poses, B)) != R360_OK) return st;
   const long long total_rays = ray_end - ray_begin;
@@ -399,7 +408,12 @@ static r360_status render_device(r360_scene* sc, const float* poses, int B, int 
   stats.chunks = chunk_idx;
   stats.kernel_launches = launches;
   sc->chunks_last = chunk_idx;
-  if (cap) { pd.chunks.clear(); pd.next = 0; }                 // a captured frame is checked with r360_graph_status
+  if (cap) {                                                   // a captured frame is checked with r360_graph_status
+    pd.chunks.clear();
+    pd.next = 0;
+    sc->graph_gen = sc->buf_gen;                               // the addresses and capacities the graph holds
+    sc->graph_live = true;
+  }
   return R360_OK;
 }
 
@@ -442,8 +456,10 @@ r360_status r360_render_batch_host_async(r360_scene* sc, const float* poses, int
     R360_CUDA(cudaMalloc(&sc->d_stage_depth[cur], R * sizeof(float)));
     sc->stage_rays_cap[cur] = R;
   }
-  // this staging set was last used two frames ago: its copy must have left before the kernels overwrite it
-  R360_CUDA(cudaStreamWaitEvent(sc->stream, sc->ev_copy_done[cur], 0));
+  // this staging set was last used two frames ago: its copy must have left before the kernels overwrite it.  A HOST
+  // wait (almost always already satisfied), so that the header's promise holds: when this call returns, the frame
+  // of the second-last call is in its host buffers
+  R360_CUDA(cudaEventSynchronize(sc->ev_copy_done[cur]));
   sc->pending.copy_done = sc->ev_copy_done[cur];
   st = render_device(sc, poses, B, W, H, 0, (long long)R, sc->d_stage_rgb[cur], sc->d_stage_depth[cur], out_rgb_host,
                      out_depth_host, sc->host_bands);
@@ -482,6 +498,8 @@ r360_status r360_wait(r360_scene* sc) {
 r360_status r360_graph_status(r360_scene* sc) {
   if (!sc) return R360_ERR_INVALID_ARG;
   R360_CUDA(cudaStreamSynchronize(sc->stream));
+  // a buffer the graph holds the address of was freed or reallocated by a later call outside the capture
+  if (sc->graph_live && sc->graph_gen != sc->buf_gen) return R360_ERR_CAPACITY;
   for (unsigned c = 0; c < sc->chunks_last; ++c)
     if (sc->h_snap[(size_t)c * 2 * kTotN]) return R360_ERR_CAPACITY;
   return R360_OK;
@@ -491,6 +509,7 @@ r360_status r360_set_graph_poses(r360_scene* sc, const float* poses, int32_t B) 
   if (!sc || !poses || B < 1 || B > sc->poses_cap || !sc->h_poses) return R360_ERR_INVALID_ARG;
   for (int i = 0; i < B * 12; ++i)
     if (!std::isfinite(poses[i])) return R360_ERR_INVALID_ARG;
+  if (sc->graph_live && sc->graph_gen != sc->buf_gen) return R360_ERR_CAPACITY;   // stale graph: capture again
   std::memcpy(sc->h_poses, poses, (size_t)B * 12 * sizeof(float));
   return R360_OK;
 }

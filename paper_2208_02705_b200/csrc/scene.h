@@ -33,6 +33,9 @@ struct r360_scene {
   float* h_poses = nullptr;                 // pinned; source of the pose copy inside a captured CUDA graph
   int poses_cap = 0;
   // chunk buffers and capacities
+  unsigned long long buf_gen = 0;           // bumped whenever a device buffer is freed or reallocated
+  unsigned long long graph_gen = 0;         // buf_gen at the last captured render call
+  bool graph_live = false;                  // a render call has been captured on this scene
   r360::ChunkBuffers buf{};
   size_t ray_cnt_cap = 0, ray_off_cap = 0, blocks_cap = 0;
   size_t seg_td_cap = 0, recs_cap = 0, out_cap_bytes = 0, dirblk_cap = 0, hit_t_cap = 0, hit_lab_cap = 0, blk_list_cap = 0, blk_list_n_cap = 0;

@@ -174,8 +174,15 @@ def test_streaming_host_output(r360, scene2):
         refs.append((rgb.cpu().numpy(), depth.cpu().numpy()))
     bufs = [(torch.empty((1, sc.H, sc.W, 3), dtype=torch.float32).pin_memory(),
              torch.empty((1, sc.H, sc.W), dtype=torch.float32).pin_memory()) for _ in poses]
-    for p, (h_rgb, h_d) in zip(poses, bufs):
+    for b in bufs:
+        b[0].fill_(-1.0); b[1].fill_(-1.0)
+    for k, (p, (h_rgb, h_d)) in enumerate(zip(poses, bufs)):
         gpu.render_batch_host(p, sc.W, sc.H, h_rgb.numpy(), h_d.numpy(), sync=False)
+        if k >= 2:
+            # include/r360.h: once the second-next call has returned, a frame is in its host buffers -- read at once,
+            # no r360_host_sync (frame 2 is the one that was re-rendered and re-copied)
+            assert np.array_equal(bufs[k - 2][0].numpy()[0], refs[k - 2][0]), k
+            assert np.array_equal(bufs[k - 2][1].numpy()[0], refs[k - 2][1]), k
     gpu.host_sync()
     assert gpu.stats().retries >= 1
     for (h_rgb, h_d), (rgb, depth) in zip(bufs, refs):
@@ -253,6 +260,76 @@ def test_cuda_graph_capture_and_replay(r360, scene2):
     del graph, g2
     gpu.close()
     gpu2.close()
+
+
+def test_stale_graph_is_reported(r360, scene2):
+    """A captured graph holds raw buffer addresses and capacities.  A later call outside the capture that frees or
+    reallocates one of them (here: a frame four times as large) makes the graph stale: r360_graph_status and
+    r360_set_graph_poses report R360_ERR_CAPACITY until the frame is captured again."""
+    import torch
+    sc = scene2
+    gpu = r360.scene_from(sc)
+    rgb = torch.zeros((1, sc.H, sc.W, 3), dtype=torch.float32, device="cuda")
+    depth = torch.zeros((1, sc.H, sc.W), dtype=torch.float32, device="cuda")
+    side = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        gpu.use_current_torch_stream()
+        ref = [t.clone() for t in gpu.render(sc.poses[0], sc.W, sc.H, rgb, depth)]
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            gpu.render(sc.poses[0], sc.W, sc.H, rgb, depth, wait=False)
+        graph.replay()
+        gpu.graph_status()
+        gpu.render(sc.poses[0], sc.W, sc.H, rgb, depth)               # same size: nothing moves, the graph stays valid
+        gpu.graph_status()
+        gpu.set_graph_poses(sc.poses[0])
+        gpu.render(sc.poses[0], 2 * sc.W, 2 * sc.H)                   # other tables, larger chunk buffers
+        torch.cuda.synchronize()
+        for call in (gpu.graph_status, lambda: gpu.set_graph_poses(sc.poses[0])):
+            with pytest.raises(r360.R360Error) as e:
+                call()
+            assert e.value.status == 6
+        gpu.render(sc.poses[0], sc.W, sc.H, rgb, depth)               # builds the tables of this size again
+        torch.cuda.synchronize()
+        g2 = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g2, stream=side):
+            gpu.render(sc.poses[0], sc.W, sc.H, rgb, depth, wait=False)
+        rgb.zero_(); depth.zero_()
+        g2.replay()
+        gpu.graph_status()
+        assert torch.equal(rgb[0], ref[0]) and torch.equal(depth[0], ref[1])
+        torch.cuda.synchronize()
+    del graph, g2
+    gpu.close()
+
+
+def test_capture_behind_an_unsettled_frame_is_refused(r360, scene2):
+    """A frame whose chunks nobody has verified (no r360_wait) may still need a re-render, which a capture cannot do
+    and would silently drop: the captured call is refused (INVALID_ARG); after r360_wait the frame is complete."""
+    import torch
+    sc = scene2
+    ref = r360.scene_from(sc)
+    want = [t.clone() for t in ref.render(sc.poses[0], sc.W, sc.H)]
+    gpu = r360.scene_from(sc)
+    side = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(side):
+        gpu.use_current_torch_stream()
+        gpu.render(_far_pose(sc), sc.W, sc.H)                          # learns a tiny capacity
+        rgb, depth = gpu.render(sc.poses[0], sc.W, sc.H, wait=False)   # overflows; not yet re-rendered
+        graph = torch.cuda.CUDAGraph()
+        with pytest.raises(r360.R360Error) as e:
+            with torch.cuda.graph(graph, stream=side, capture_error_mode="thread_local"):
+                gpu.render(sc.poses[0], sc.W, sc.H, rgb, depth, wait=False)
+        assert e.value.status == 1
+        gpu.wait()
+        torch.cuda.synchronize()
+        assert gpu.stats().retries == 1
+        assert torch.equal(rgb, want[0]) and torch.equal(depth, want[1])
+    gpu.close()
+    ref.close()
 
 
 def test_capture_of_a_cold_scene_is_refused(r360, scene1):
