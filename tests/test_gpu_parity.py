@@ -284,3 +284,78 @@ def test_more_subfields_than_the_shared_memory_histogram_holds(r360, oracle):
     check_image(rgb.cpu().numpy(), depth.cpu().numpy(), ref, 2e-3, amb_band=AMB_BAND["bf16"], depth_tol=2e-3 * t_max)
     gpu.close()
     ora.close()
+
+
+def _rows_bit_exact(gpu, ora, pose, W, H, rows):
+    """Whole-image layout check plus (count, t bits, subfield id) of every sample of the given rows against the
+    oracle; the sample arrays stay on the device (hundreds of millions of samples), only the rows' entries come back.
+    Returns the per-ray counts [H, W]."""
+    import torch
+    counts, offsets, t, sid = gpu.debug_samples(pose, W, H)
+    c = counts.cpu().numpy().view(np.uint32).astype(np.int64)
+    o = offsets.cpu().numpy().view(np.uint32).astype(np.int64)
+    total = int(c.sum())
+    assert total == t.numel() == sid.numel()
+    # the per-ray ranges [offset, offset + count) are disjoint and cover [0, total), in any ray order
+    live = np.flatnonzero(c)
+    order = live[np.argsort(o[live], kind="stable")]
+    assert o[order[0]] == 0 and np.array_equal(o[order[1:]], (o[order] + c[order])[:-1])
+    assert o[order[-1]] + c[order[-1]] == total
+    c, o = c.reshape(H, W), o.reshape(H, W)
+    t_bits = t.view(torch.int32)
+    rows = sorted({int(np.unravel_index(int(c.argmax()), c.shape)[0]) if r == "longest" else r for r in rows})
+    for row in rows:
+        oc, ot, osid = ora.samples_rows(pose, W, H, row, row + 1)
+        assert np.array_equal(c[row], oc), row                                   # bit-exact counts
+        oc64 = oc.astype(np.int64)
+        idx = np.repeat(o[row], oc64) + (np.arange(int(oc64.sum())) - np.repeat(np.cumsum(oc64) - oc64, oc64))
+        idx = torch.from_numpy(idx).cuda()
+        assert np.array_equal(t_bits[idx].cpu().numpy(), ot.view(np.int32)), row  # bit-exact distances
+        assert np.array_equal(sid[idx].cpu().numpy(), osid), row                  # exact subfield ids
+    return c, rows
+
+
+def test_sampler_bit_exact_config5_rows(r360, oracle):
+    """BASELINE config 5 (30 % occupancy) at full size: rows 0, H/2, H-1 and the row of the longest ray, every sample.
+    Rays that cross more than kHitCap = 64 occupied voxels leave k_count's per-ray hit buffer and are walked again
+    by k_emit (sampler.cu): at least one compared ray must be of that kind, so that branch is held to the oracle
+    bit for bit and not only through an image tolerance (north_star: counts and ids bit-exact)."""
+    sc = get_scene(5)
+    gpu = r360.scene_from(sc)
+    ora = oracle.scene_from(sc)
+    K = sc.samples_per_voxel
+    c, rows = _rows_bit_exact(gpu, ora, sc.poses[0], sc.W, sc.H, (0, sc.H // 2, sc.H - 1, "longest"))
+    segs = c[rows] // K
+    assert segs.max() > 64 and (segs > 64).sum() >= 10, "no compared ray takes the re-walk branch"
+    rgb, depth = gpu.render(sc.poses[0], sc.W, sc.H)
+    assert gpu.stats().samples_emitted == int(c.sum())                           # the render agrees with the tap
+    gpu.close()
+    ora.close()
+
+
+def test_sampler_bit_exact_config4_rows_and_pose_boundary(r360, oracle):
+    """BASELINE config 4 (512 x 512 x 96 grid: skip distances saturate at 255; K = 12; 4096 x 2048): three rows of
+    pose 3, every sample; then two poses in one batch with a ray chunk that straddles the pose boundary, each image
+    equal bit for bit to its single render."""
+    import torch
+    sc = get_scene(4)
+    gpu = r360.scene_from(sc)
+    ora = oracle.scene_from(sc)
+    assert sc.samples_per_voxel == 12 and tuple(sc.dims) == (512, 512, 96)
+    _rows_bit_exact(gpu, ora, sc.poses[3], sc.W, sc.H, (0, sc.H // 2, sc.H - 1))
+    ora.close()
+    gpu.set_precision("bf16")
+    singles = []
+    for p in (sc.poses[3], sc.poses[4]):
+        rgb, depth = gpu.render(p, sc.W, sc.H)
+        singles.append((rgb.clone(), depth.clone()))
+    assert gpu.stats().samples_emitted > 0
+    rays = sc.W * sc.H
+    gpu.set_chunk_rays(3 << 20)                                                  # chunk 2 = rays [6 Mi, 9 Mi): both poses
+    assert (2 * (3 << 20)) < rays < (3 * (3 << 20))
+    rgb2, d2 = gpu.render_batch(np.stack([sc.poses[3], sc.poses[4]]), sc.W, sc.H)
+    assert gpu.stats().chunks == (2 * rays + (3 << 20) - 1) // (3 << 20)
+    for b in range(2):
+        assert torch.equal(rgb2[b], singles[b][0]) and torch.equal(d2[b], singles[b][1])
+    assert not torch.equal(rgb2[0], rgb2[1])
+    gpu.close()

@@ -109,6 +109,12 @@ def test_render_tc_width64(r360, oracle, prec):
 
 
 BF16_SINGLE_SAMPLE_BOUND = 4e-3
+# Rays inside the threshold-ambiguity band (reading G4; gpu_util.check_image) are held to an interval that is at most
+# tau * max|rgb| = 1e-3 wider than the tolerance, not to the tolerance itself: on the opaque scenes they must stay a
+# minority, or the image comparison would say little.  Measured on the density-bias-40 scene (T falls by e^-1.25 per
+# sample, so the threshold is crossed between two samples of most rays): 233 of 2048 rays (11.4 %) lie inside
+# bfloat16's band of 0.06, 74 (3.6 %) inside binary16's 0.02; none on the saturating-density scenes.
+MAX_AMBIGUOUS_FRACTION = {"bf16": 0.15, "f16": 0.05}
 
 
 def test_bfloat16_operands_on_opaque_scenes_stay_within_their_format_limit(r360, oracle, scene1):
@@ -120,12 +126,15 @@ def test_bfloat16_operands_on_opaque_scenes_stay_within_their_format_limit(r360,
     asserted is that format limit with margin, 4e-3; the mode that meets 2e-3 on these scenes is binary16 operands
     (test_render_f16_opaque_scenes below: 3.3e-4 / 4.5e-4).  On all five BASELINE.json configs, where a pixel
     averages 35-290 samples, mode 1 is within 2e-3 (tests above and below)."""
+    n_rays = scene1.W * scene1.H
     e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 40.0), tol=BF16_SINGLE_SAMPLE_BOUND)
-    print("dense stress bf16 max rgb err", e_rgb)
+    print("dense stress bf16 max rgb err", e_rgb, "ambiguous", n_amb, "of", n_rays)
+    assert n_amb <= MAX_AMBIGUOUS_FRACTION["bf16"] * n_rays
     for act in (0, 1):
         e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 1.0e6),
                                  tol=BF16_SINGLE_SAMPLE_BOUND, density_activation=act)
-        print("saturating density bf16 act", act, "max rgb err", e_rgb)
+        print("saturating density bf16 act", act, "max rgb err", e_rgb, "ambiguous", n_amb, "of", n_rays)
+        assert n_amb <= MAX_AMBIGUOUS_FRACTION["bf16"] * n_rays
 
 
 def test_render_f16_opaque_scenes(r360, oracle, scene1):
@@ -133,13 +142,16 @@ def test_render_f16_opaque_scenes(r360, oracle, scene1):
     north_star's bar, 2e-3, on the binary16-operand tensor path: density bias 40 (every pixel is the colour of its
     first one or two samples) and density far beyond binary16's range (sigma stored clamped to 65504, alpha = 1).
     Ambiguity band: gpu_util.AMB_BAND."""
+    n_rays = scene1.W * scene1.H
     e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 40.0),
                              tol=TOL, precision="f16")
-    print("dense stress f16 max rgb err", e_rgb, "ambiguous", n_amb)
+    print("dense stress f16 max rgb err", e_rgb, "ambiguous", n_amb, "of", n_rays)
+    assert n_amb <= MAX_AMBIGUOUS_FRACTION["f16"] * n_rays
     for act in (0, 1):
         e_rgb, e_d, n_amb = _cmp(r360, oracle, scene1, weights=with_density_bias(scene1, 1.0e6),
                                  tol=TOL, density_activation=act, precision="f16")
-        print("saturating density f16 act", act, "max rgb err", e_rgb)
+        print("saturating density f16 act", act, "max rgb err", e_rgb, "ambiguous", n_amb, "of", n_rays)
+        assert n_amb <= MAX_AMBIGUOUS_FRACTION["f16"] * n_rays
 
 
 def test_f16_refused_when_a_weight_exceeds_binary16(r360, scene1):
