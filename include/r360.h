@@ -96,11 +96,15 @@ void r360_scene_destroy(r360_scene* scene);
 /* Render one W x H view with the scene's camera (r360_set_camera; default: the equirectangular panorama of
  * Eq. 2-3) -- Eq. 2-5; steps a1-a10 of DESIGN.md.
  *  pose       HOST float[12]: row-major 3x4 [R|o], camera (x right, y down, z forward,
- *             PAPER.md:84) -> world; o = camera centre.  Must be finite.
+ *             PAPER.md:84) -> world; o = camera centre.  Must be finite, and R must not be (nearly) singular:
+ *             2^-16 <= ||R||_F <= 2^16 and |det R| >= 2^-16 ||R||_F^3, evaluated in binary64 (DESIGN.md reading
+ *             B5).  Every rotation passes, with or without a moderate scale; a matrix that maps some unit
+ *             direction of Eq. 3 to (nearly) zero does not.  The same rule holds for every pose argument of
+ *             this header (batches, graph poses, the fusion calls, the debug taps).
  *  out_rgb    DEVICE float[H*W*3], row-major, black background   (R360_OUT_RGB8_D16: uint8[H*W*3])
  *  out_depth  DEVICE float[H*W], Eq. 4's sum w_i t_i (radial distance; not opacity-normalised)
  *             (R360_OUT_RGB8_D16: binary16[H*W])
- * Asynchronous (see "Conventions").  Errors: INVALID_ARG (NULL, W < 1, H < 1, non-finite pose), OOM, CUDA;
+ * Asynchronous (see "Conventions").  Errors: INVALID_ARG (NULL, W < 1, H < 1, non-finite or singular pose), OOM, CUDA;
  * CAPACITY inside a CUDA stream capture when a buffer would have to be allocated (see r360_graph_status). */
 r360_status r360_render(r360_scene* scene, const float pose[12], int32_t W, int32_t H,
                         void* out_rgb, void* out_depth);

@@ -206,6 +206,8 @@ class OracleScene:
         pose = np.ascontiguousarray(pose, np.float32).reshape(12)
         t = np.empty(cap, np.float32); dl = np.empty(cap, np.float32); sid = np.empty(cap, np.int32)
         n = self.o.lib.r360o_ray_samples(self.h, _p(pose, _F), W, H, i, j, cap, _p(t, _F), _p(dl, _F), _p(sid, _I))
+        if n == -2:
+            raise ValueError("r360o_ray_samples: inadmissible pose (reading B5)")
         assert n <= cap
         return t[:n].copy(), dl[:n].copy(), sid[:n].copy()
 
@@ -215,6 +217,8 @@ class OracleScene:
         row1 = H if row1 is None else row1
         counts = np.empty((row1 - row0) * W, np.uint32)
         total = self.o.lib.r360o_samples_rows(self.h, _p(pose, _F), W, H, row0, row1, _p(counts, _U), 0, None, None)
+        if total == -2:
+            raise ValueError("r360o_samples_rows: inadmissible pose (reading B5)")
         t = np.empty(max(total, 1), np.float32); sid = np.empty(max(total, 1), np.int32)
         got = self.o.lib.r360o_samples_rows(self.h, _p(pose, _F), W, H, row0, row1, _p(counts, _U), total,
                                             _p(t, _F), _p(sid, _I))

@@ -300,6 +300,9 @@ typedef void (*visit_fn)(void* ctx, int64_t voxel, float t_in, float t_out, int 
 /* C3-C4: walk, calling visit() for every crossed voxel (t_in < t_out, strict). */
 static void walk(const r360o_scene* s, const ray_t* r, visit_fn visit, void* ctx) {
   float t0, t1;
+  /* a direction with no component of 2^-100 or more (reading C1 makes every axis parallel) goes nowhere: it crosses
+   * no voxel boundary and there is no exit axis to step along (reading B5 keeps such rays out of the render calls) */
+  if (r->par[0] && r->par[1] && r->par[2]) return;
   if (!clip(s, r, &t0, &t1)) return;
   int idx[3];
   for (int a = 0; a < 3; ++a) {                       /* C3 */
@@ -391,9 +394,29 @@ static int64_t ray_samples(const r360o_scene* s, const float o[3], const float d
   return c.n;
 }
 
+/* Reading B5: a pose is admissible iff its 12 entries are finite and its 3x3 part M, taken in binary64,
+ * has 2^-16 <= |M|_F <= 2^16 and |det M| >= 2^-16 |M|_F^3.  Every rotation passes (|det| / |M|_F^3 = 3^-1.5 = 0.19),
+ * also with a moderate scale; a singular or nearly singular M, which maps some unit camera direction of Eq. 3 to
+ * (nearly) zero, does not: the smallest singular value of an admissible M is at least |det| / |M|_F^2 >=
+ * 2^-16 |M|_F, far above the rounding of reading B3's three products and two sums (about 2^-22 |M|_F). */
+int r360o_pose_ok(const float pose[12]) {
+  if (!pose) return 0;
+  for (int a = 0; a < 12; ++a) if (!isfinite(pose[a])) return 0;
+  double m[3][3], f2 = 0.0;
+  for (int a = 0; a < 3; ++a)
+    for (int b = 0; b < 3; ++b) { m[a][b] = (double)pose[a * 4 + b]; f2 += m[a][b] * m[a][b]; }
+  double f = sqrt(f2);
+  double det = m[0][0] * (m[1][1] * m[2][2] - m[1][2] * m[2][1]) - m[0][1] * (m[1][0] * m[2][2] - m[1][2] * m[2][0]) +
+               m[0][2] * (m[1][0] * m[2][1] - m[1][1] * m[2][0]);
+  const double lim = 1.0 / 65536.0;
+  if (!(f >= lim && f <= 65536.0)) return 0;
+  return fabs(det) >= lim * f * f * f;
+}
+
 int64_t r360o_ray_samples(const r360o_scene* s, const float pose[12], int32_t W, int32_t H,
                           int32_t i, int32_t j, int64_t cap, float* t, float* delta, int32_t* subfield) {
   float o[3], d[3];
+  if (!r360o_pose_ok(pose)) return -2;
   if (s->cam_model == 1) r360o_ray_pinhole(pose, s->fx, s->fy, s->cx, s->cy, i, j, o, d);
   else r360o_ray(pose, W, H, i, j, o, d);
   return ray_samples(s, o, d, cap, t, delta, subfield);
@@ -579,7 +602,7 @@ int r360o_render_pixels(const r360o_scene* s, const float pose[12], int32_t W, i
                         float* rgb, float* depth, float* rgb_full, float* depth_full,
                         float* ambiguity, uint32_t* n_emitted, uint32_t* n_used) {
   if (!s || !pose || W < 1 || H < 1 || n_pix < 0) return 1;
-  for (int a = 0; a < 12; ++a) if (!isfinite(pose[a])) return 1;
+  if (!r360o_pose_ok(pose)) return 1;                        /* B5 */
   float* tab = camera_tables(s, W, H);
   int bad = 0;
 #pragma omp parallel for schedule(dynamic, 64)
@@ -597,7 +620,7 @@ int r360o_render_rows(const r360o_scene* s, const float pose[12], int32_t W, int
                       float* rgb, float* depth, float* rgb_full, float* depth_full,
                       float* ambiguity, uint32_t* n_emitted, uint32_t* n_used) {
   if (!s || !pose || W < 1 || H < 1 || row0 < 0 || row1 > H || row0 > row1) return 1;
-  for (int a = 0; a < 12; ++a) if (!isfinite(pose[a])) return 1;
+  if (!r360o_pose_ok(pose)) return 1;                        /* B5 */
   float* tab = camera_tables(s, W, H);
   int64_t n_pix = (int64_t)(row1 - row0) * W;
 #pragma omp parallel for schedule(dynamic, 64)
@@ -615,6 +638,7 @@ int r360o_render_rows(const r360o_scene* s, const float pose[12], int32_t W, int
 int64_t r360o_samples_rows(const r360o_scene* s, const float pose[12], int32_t W, int32_t H,
                            int32_t row0, int32_t row1, uint32_t* counts, int64_t cap, float* t,
                            int32_t* subfield) {
+  if (!r360o_pose_ok(pose)) return -2;                       /* B5 */
   int64_t n_pix = (int64_t)(row1 - row0) * W;
   float* tab = camera_tables(s, W, H);
   float o[3] = {pose[3], pose[7], pose[11]};

@@ -83,6 +83,10 @@ int64_t r360o_walk(const r360o_scene* s, const float o[3], const float d[3], int
 /* Box clip (C2): returns 1 and [t0,t1] if the ray has a non-empty interval. */
 int r360o_clip(const r360o_scene* s, const float o[3], const float d[3], float* t0, float* t1);
 
+/* Reading B5: 1 iff the pose is admissible (finite; 3x3 part M with 2^-16 <= |M|_F <= 2^16 and
+ * |det M| >= 2^-16 |M|_F^3 in binary64).  The render / sample functions below return an error (1, or -2 where they
+ * return a count) for any other pose. */
+int r360o_pose_ok(const float pose[12]);
 /* Samples of one pixel's ray (reading D). Returns count (may exceed cap). */
 int64_t r360o_ray_samples(const r360o_scene* s, const float pose[12], int32_t W, int32_t H,
                           int32_t i, int32_t j, int64_t cap, float* t, float* delta, int32_t* subfield);

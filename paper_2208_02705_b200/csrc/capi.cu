@@ -73,6 +73,32 @@ void transpose_layer(const float* src, float* dst, int out, int in, int out_pad)
 
 }  // namespace
 
+// DESIGN.md reading B5: B poses are admissible iff every entry is finite and every 3x3 part R (binary64) satisfies
+// 2^-16 <= ||R||_F <= 2^16 and |det R| >= 2^-16 ||R||_F^3.  A rotation gives 3^-1.5; a (nearly) singular R would map
+// some unit direction of Eq. 3 to (nearly) zero, a "ray" that has no exit face in the walk.
+bool r360_poses_ok(const float* poses, int B) {
+  if (!poses || B < 1) return false;
+  for (int b = 0; b < B; ++b) {
+    const float* P = poses + (size_t)b * 12;
+    double r[9], sq = 0.0;
+    for (int i = 0; i < 12; ++i)
+      if (!std::isfinite(P[i])) return false;
+    for (int row = 0; row < 3; ++row)
+      for (int col = 0; col < 3; ++col) {
+        const double v = (double)P[row * 4 + col];
+        r[row * 3 + col] = v;
+        sq += v * v;
+      }
+    const double nf = std::sqrt(sq);
+    if (!(nf >= 0x1p-16 && nf <= 0x1p16)) return false;
+    // det by the rule of Sarrus
+    const double det = r[0] * r[4] * r[8] + r[1] * r[5] * r[6] + r[2] * r[3] * r[7] - r[2] * r[4] * r[6] -
+                       r[1] * r[3] * r[8] - r[0] * r[5] * r[7];
+    if (!(std::fabs(det) >= 0x1p-16 * nf * nf * nf)) return false;
+  }
+  return true;
+}
+
 r360_status r360_cuda_fail(cudaError_t e, const char* what) {
   snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
   cudaGetLastError();  // clear the non-sticky error state

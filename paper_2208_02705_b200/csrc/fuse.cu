@@ -197,8 +197,7 @@ r360_status r360_fusion_fuse_device(r360_fusion* fu, const float pose[12], int32
                                     const float* uncertainty) {
   if (!fu || !pose || !depth || W < 1 || H < 1) return R360_ERR_INVALID_ARG;
   if ((long long)W * H >= (1ll << 30)) return R360_ERR_INVALID_ARG;
-  for (int i = 0; i < 12; ++i)
-    if (!std::isfinite(pose[i])) return R360_ERR_INVALID_ARG;
+  if (!r360_poses_ok(pose, 1)) return R360_ERR_INVALID_ARG;     // non-finite or (nearly) singular (reading B5)
   if (!fu->d_tab || fu->tab_W != W || fu->tab_H != H) {
     // reading B2: trig of the pixel-centre angles in binary64, rounded once
     const double kPi = 3.14159265358979323846;
@@ -348,8 +347,7 @@ extern "C" r360_status r360_fusion_fuse_static(const int32_t dims[3], const floa
     g.vs[a] = ext / (float)dims[a];
     g.inv_vs[a] = 1.0f / g.vs[a];
   }
-  for (int i = 0; i < 12; ++i)
-    if (!std::isfinite(pose[i])) return R360_ERR_INVALID_ARG;
+  if (!r360_poses_ok(pose, 1)) return R360_ERR_INVALID_ARG;     // non-finite or (nearly) singular (reading B5)
   const unsigned long long N64 = (unsigned long long)dims[0] * (unsigned long long)dims[1] * (unsigned long long)dims[2];
   if (N64 > kStaticMaxVoxels || W > kStaticMaxW || H > kStaticMaxH) {
     // the text r360_last_cuda_error() returns names the limit that was hit

@@ -85,8 +85,7 @@ r360_status ensure_tables(r360_scene* sc, int W, int H) {
 }
 
 r360_status upload_poses(r360_scene* sc, const float* poses, int B) {
-  for (int i = 0; i < B * 12; ++i)
-    if (!std::isfinite(poses[i])) return R360_ERR_INVALID_ARG;
+  if (!r360_poses_ok(poses, B)) return R360_ERR_INVALID_ARG;   // non-finite, or a (nearly) singular 3x3 part (B5)
   const bool cap = capturing(sc->stream);
   if (B > sc->poses_cap) {
     if (cap) return R360_ERR_CAPACITY;
@@ -507,8 +506,7 @@ r360_status r360_graph_status(r360_scene* sc) {
 
 r360_status r360_set_graph_poses(r360_scene* sc, const float* poses, int32_t B) {
   if (!sc || !poses || B < 1 || B > sc->poses_cap || !sc->h_poses) return R360_ERR_INVALID_ARG;
-  for (int i = 0; i < B * 12; ++i)
-    if (!std::isfinite(poses[i])) return R360_ERR_INVALID_ARG;
+  if (!r360_poses_ok(poses, B)) return R360_ERR_INVALID_ARG;
   if (sc->graph_live && sc->graph_gen != sc->buf_gen) return R360_ERR_CAPACITY;   // stale graph: capture again
   std::memcpy(sc->h_poses, poses, (size_t)B * 12 * sizeof(float));
   return R360_OK;

@@ -86,6 +86,9 @@ struct r360_scene {
 // render.cu: verify the chunks of the last render call, re-render what overflowed (block: wait for their k_scan)
 r360_status r360_settle(r360_scene* sc, bool block);
 
+// capi.cu: reading B5 -- finite, and every 3x3 part well conditioned (no unit direction is mapped to ~zero)
+bool r360_poses_ok(const float* poses, int B);
+
 // records the CUDA error text for r360_last_cuda_error() and maps it to a status
 r360_status r360_cuda_fail(cudaError_t e, const char* what);
 

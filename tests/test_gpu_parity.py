@@ -167,6 +167,19 @@ def test_render_rejects_bad_arguments(r360, scene1):
     assert e.value.status == 1
     L = r360.lib()
     assert L.r360_render(gpu._h, None, 64, 32, None, None) == 1
+    # reading B5: a (nearly) singular 3x3 part maps some pixel's unit direction to ~zero -- refused by both sides
+    for scale_z in (0.0, 1e-7):
+        flat = scene1.poses[0].copy().reshape(3, 4)
+        flat[:, 2] *= scale_z
+        with pytest.raises(r360.R360Error) as e:
+            gpu.render(flat.reshape(12), 64, 32)
+        assert e.value.status == 1
+        with pytest.raises(r360.R360Error):
+            gpu.render_batch(np.stack([scene1.poses[0], flat.reshape(12)]), 64, 32)
+        with pytest.raises(r360.R360Error):
+            gpu.debug_samples(flat.reshape(12), 64, 32)
+    rgb, depth = gpu.render(scene1.poses[0] * np.array([2, 2, 2, 1] * 3, F), 64, 32)   # a scaled rotation is fine
+    assert float(depth.max()) > 0
 
 
 def test_full_size_config3_sampled(r360, oracle):
