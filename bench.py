@@ -3,7 +3,8 @@
 equirect render of config 3 (multi-room floor, ~1k subfields); MLP samples/s and roofline fraction.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 3]
-                  [--precision auto|fp32|bf16|f16] [--scaling weak|strong]
+                  [--precision auto|fp32|bf16|f16] [--scaling weak|strong] [--no-other-configs]
+                  [--no-paper-conditions] [--all-configs]
 
 A step = one whole pass of the hot path (ray generation, occupancy walk, binning, grouped tiny
 MLP, compositing) over one frame of synthetic input (scenegen, seeded).
@@ -42,12 +43,13 @@ def executed_flop_per_sample(width, n_hidden, pe_p=63, pe_d=27):
     return flop_per_sample(width, n_hidden, pe_p, pe_d) - 2 * width * width
 
 
-def ncu_traffic(kernel):
-    """DRAM bytes (read + write) of one launch of `kernel` on config 3 / bf16, from the committed ncu --set full
-    capture (profiles/traffic.json names the capture and the CSV rows it was read from); None if not recorded."""
+def ncu_traffic(kernel, config=3):
+    """DRAM bytes (read + write) of ONE launch of `kernel` on `config` / bf16, from the committed ncu --set full
+    captures (profiles/traffic.json names each capture, the CSV rows it was read from and what one launch covers:
+    a whole frame on configs 3 and 5, ray chunk 0 of pose 0 on config 4); None if not recorded."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     try:
-        return json.load(open(p)).get(kernel)
+        return json.load(open(p)).get(str(config), {}).get(kernel)
     except (OSError, ValueError):
         return None
 
@@ -220,7 +222,7 @@ def mlp_roofline(sc, precision, samples, ms_mlp, peaks, alu_peak):
             "samples_per_launch": int(samples), "ms_per_launch": ms_mlp}
 
 
-def hbm_stage_table(sc, precision, W, H, B, segs, stage_med, peaks, with_traffic):
+def hbm_stage_table(sc, precision, W, H, B, segs, stage_med, peaks, with_traffic, launches=1):
     """The memory-side stages against the measured HBM copy bandwidth: algorithmic bytes."""
     rays, Kk = W * H * B, sc.samples_per_voxel
     tensor = precision != "fp32"
@@ -235,7 +237,13 @@ def hbm_stage_table(sc, precision, W, H, B, segs, stage_med, peaks, with_traffic
         ms_k = stage_med[stage_key[kname]]
         gbs = nbytes / (ms_k * 1e-3) / 1e9 if ms_k > 0 else 0.0
         out[kname] = {"algorithmic_bytes": int(nbytes), "ms": ms_k, "achieved_gbs": gbs,
-                      "frac_of_hbm_peak": gbs / peaks["hbm"], "traffic": ncu_traffic(kname) if with_traffic else None}
+                      "frac_of_hbm_peak": gbs / peaks["hbm"],
+                      "traffic": ncu_traffic(kname, sc.config) if with_traffic else None}
+        if with_traffic and launches > 1:
+            # algorithmic_bytes and ms cover the step's `launches` launches of this kernel (one per ray chunk);
+            # `traffic` is the ncu figure of ONE of them (profiles/traffic.json says which)
+            out[kname]["launches_per_step"] = launches
+            out[kname]["algorithmic_bytes_per_launch_mean"] = int(nbytes / launches)
     return out
 
 
@@ -249,7 +257,9 @@ def time_config(r360, config, precision, peaks, alu_peak, steps=5, warmup=3, pin
     import torch
     from scenegen import make_scene
     sc = make_scene(config)
-    scene = r360.scene_from(sc)
+    t_create = time.perf_counter()
+    scene = r360.scene_from(sc)          # r360_scene_create: uploads, label check, octant skip table (host), weight packing
+    t_create = time.perf_counter() - t_create
     scene.set_precision(precision)
     scene.use_current_torch_stream()
     W, H = sc.W, sc.H
@@ -287,8 +297,13 @@ def time_config(r360, config, precision, peaks, alu_peak, steps=5, warmup=3, pin
            "fps": B * 1e3 / med, "samples_per_step": int(st.samples_emitted), "segments_per_step": int(st.segments),
            "mlp_samples_per_s": st.samples_emitted / (stage_med["ms_mlp"] * 1e-3) if stage_med["ms_mlp"] > 0 else None,
            "stage_ms": stage_med, "chunks": int(st.chunks), "kernel_launches": int(st.kernel_launches),
+           "scene_create_s": t_create,
            "roofline": mlp_roofline(sc, precision, st.samples_emitted, stage_med["ms_mlp"], peaks, alu_peak),
-           "hbm_stages": hbm_stage_table(sc, precision, W, H, B, int(st.segments), stage_med, peaks, False)}
+           "hbm_stages": hbm_stage_table(sc, precision, W, H, B, int(st.segments), stage_med, peaks,
+                                         precision == "bf16" and not pinhole and not stereo, launches=int(st.chunks))}
+    if precision == "bf16" and not pinhole and not stereo:
+        out["roofline"]["traffic"] = ncu_traffic("k_mlp_tc", config)
+        out["roofline"]["traffic_note"] = "ncu, one launch (profiles/traffic.json); this step has %d" % int(st.chunks)
     scene.close()
     del rgb, depth, flush
     torch.cuda.empty_cache()
@@ -326,7 +341,21 @@ def time_extras(r360, config):
     L0 = np.zeros(int(np.prod(sc.dims)), np.float32)
     dt, L = wall(lambda: r360.occupancy_fuse(L0, sc.dims, sc.box_min, sc.box_max, sc.poses[0], W, H, depth), 5)
     out["occupancy_fuse"] = {"seconds": dt, "image": [W, H], "voxels": int(L0.size), "voxels_updated": int((L != 0).sum()),
-                             "what": "one observation of Eq. 6 (PAPER.md:117-128), r360_occupancy_fuse, synthetic depth"}
+                             "what": "one observation of Eq. 6 (PAPER.md:117-128), r360_occupancy_fuse (host grid in and "
+                                     "out: create + copy + fuse + read + destroy), synthetic depth"}
+    # the same observation with everything resident on the device (Algorithm 1 stage I fuses panoramas progressively)
+    d_depth = torch.from_numpy(depth).cuda()
+    fu = r360.Fusion(sc.dims, sc.box_min, sc.box_max)
+    dt, _ = wall(lambda: fu.fuse(sc.poses[0], W, H, d_depth), 20)
+    fu.close()
+    out["fusion_fuse_device"] = {"seconds": dt, "image": [W, H], "voxels": int(L0.size),
+                                 "what": "r360_fusion_fuse_device: grid and depth image resident on the device"}
+    if L0.size <= r360.STATIC_MAX_VOXELS:
+        d_L = torch.zeros(L0.size, device="cuda")
+        dt, _ = wall(lambda: r360.fusion_fuse_static(d_L, sc.dims, sc.box_min, sc.box_max, sc.poses[0], W, H, d_depth), 20)
+        out["fusion_fuse_static"] = {"seconds": dt, "image": [W, H], "voxels": int(L0.size),
+                                     "what": "r360_fusion_fuse_static: the same without any allocation (static scratch, "
+                                             "cleared per call)"}
     return out
 
 
@@ -343,8 +372,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true",
                     help="skip the short device-timed entries of configs 4, 5 and of this config's other precisions")
-    ap.add_argument("--all-configs", action="store_true",
-                    help="also time configs 1, 2, the 720p pinhole view, a stereo pair and the stand-alone entry points")
+    ap.add_argument("--no-paper-conditions", action="store_true",
+                    help="skip the 720p pinhole views (the paper's timing condition), the stereo pair and the "
+                         "stand-alone entry points (SURVEY.md 8(f))")
+    ap.add_argument("--all-configs", action="store_true", help="also time configs 1 and 2")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -361,12 +392,15 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     import __graft_entry__ as g
     import paper_2208_02705_b200 as r360
-    if not os.path.exists(r360.lib_path()):
+    from paper_2208_02705_b200 import build as _build
+    if not (os.path.exists(r360.lib_path()) and os.path.exists(_build.BENCH_SO)):
         g.build()
     from paper_2208_02705_b200.shard import rank_pose, render_sharded
     from scenegen import make_scene
     sc = make_scene(args.config)
+    scene_create_s = time.perf_counter()
     scene = r360.scene_from(sc)
+    scene_create_s = time.perf_counter() - scene_create_s
     precision = args.precision
     if precision == "auto":
         try:
@@ -482,14 +516,14 @@ def main():
     if rank == 0:
         peaks = measured_peaks()
         tf, mhz = r360.measure_fp32_fma()
-        alu_peak = {"tflops": tf, "source": f"measured on this GPU: r360_measure_fp32_fma (register-only FMA kernel, "
+        alu_peak = {"tflops": tf, "source": f"measured on this GPU: r360bench_fp32_fma in libr360_bench.so (register-only FMA kernel, "
                                             f"best of 5), nominal SM clock {mhz:.0f} MHz"}
         samples = st.samples_emitted
         stage_med = {k: statistics.median(v) for k, v in stage.items()}
         roof = mlp_roofline(sc, precision, samples, stage_med["ms_mlp"], peaks, alu_peak)
-        on_capture = precision == "bf16" and args.config == 3 and not strong     # what the committed ncu capture ran
+        on_capture = precision == "bf16" and not strong                          # what the committed ncu captures ran
         if on_capture:
-            roof["traffic"] = ncu_traffic("k_mlp_tc")
+            roof["traffic"] = ncu_traffic("k_mlp_tc", args.config)
         line = {"metric": "rays_per_second_equirect_render", "value": value, "unit": "rays/s", "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step, "ms_per_step_median": ms_median,
                 "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
@@ -502,7 +536,7 @@ def main():
                                                         "(r360_get_stats), rank 0",
                 "clocks": clk, "roofline": roof,
                 "hbm_stages": hbm_stage_table(sc, precision, W, H if not strong else -(-H // world), 1, int(st.segments),
-                                              stage_med, peaks, on_capture),
+                                              stage_med, peaks, on_capture, launches=int(st.chunks)),
                 "e2e": e2e, "e2e_rgb8_d16": e2e_small, "e2e_stream_of_frames": e2e_stream,
                 "gpu_launches": int(launches), "retries": int(st.retries)}
         scene.close()
@@ -515,14 +549,26 @@ def main():
             others += [time_config(r360, c, "bf16", peaks, alu_peak, steps=3 if c == 4 else 5) for c in (4, 5)
                        if c != args.config]
             line["other_configs"] = others
-        if args.all_configs:
-            more = [time_config(r360, c, precision, peaks, alu_peak) for c in (1, 2) if c != args.config]
-            # the paper times its perspective (roaming) view at 720p: same scene, 90 degree pinhole
-            more.append(time_config(r360, args.config, precision, peaks, alu_peak, pinhole=(1280, 720, 640.0)))
-            # stereoscopic mode: two eyes in one batch, against two mono frames
-            more.append(time_config(r360, args.config, precision, peaks, alu_peak, stereo=True))
-            line["more_configs"] = more
+        if not args.no_paper_conditions:
+            # SURVEY.md 8(f) rows and the paper's own timing condition, device-timed, a few steps each.
+            # The paper times its perspective (roaming) view at 720p (Fig. 8 :216 at n = 2048): the same
+            # scenes through a 90 degree pinhole camera -- this config and config 5's 2048-subfield scene.
+            pc = [time_config(r360, args.config, precision, peaks, alu_peak, steps=5, pinhole=(1280, 720, 640.0))]
+            if args.config != 5:
+                pc.append(time_config(r360, 5, "bf16", peaks, alu_peak, steps=5, pinhole=(1280, 720, 640.0)))
+            # stereoscopic mode: two eyes in one batch, against two mono frames of the main run
+            stereo = time_config(r360, args.config, precision, peaks, alu_peak, steps=5, stereo=True)
+            stereo["two_mono_frames_ms"] = 2.0 * ms_median
+            stereo["pair_over_two_mono"] = stereo["ms_per_step"] / (2.0 * ms_median)
+            pc.append(stereo)
+            line["paper_conditions"] = pc
             line["extras"] = time_extras(r360, args.config)
+        # what r360_scene_create costs (host work: label check, octant skip table, weight packing; uploads)
+        line["scene_create_s"] = {str(args.config): scene_create_s}
+        for o in line.get("other_configs", []) + line.get("paper_conditions", []):
+            line["scene_create_s"].setdefault(str(o["config"]), o["scene_create_s"])
+        if args.all_configs:
+            line["more_configs"] = [time_config(r360, c, precision, peaks, alu_peak) for c in (1, 2) if c != args.config]
         if not args.no_cpu_baseline:
             cb = oracle_sample(sc, args.ref_row_stride)
             line["cpu_baseline"] = {"value": cb["rays_per_s"], "unit": "rays/s", "cores": cb["cores"],

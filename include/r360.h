@@ -336,11 +336,6 @@ r360_status r360_debug_samples(r360_scene* scene, const float pose[12], int32_t 
                                uint32_t* counts, uint32_t* offsets, float* t, int32_t* subfield,
                                uint64_t cap, uint64_t* total);
 
-/* Measurement helper for bench.py: the FP32 FMA rate of the current device in TFLOP/s (2 FLOP per FMA; best of five
- * launches of a register-only FMA kernel that fills every SM), the roofline of the fp32 MLP path.
- * sm_mhz_out (may be NULL) receives the device's nominal SM clock. */
-r360_status r360_measure_fp32_fma(double* tflops_out, double* sm_mhz_out);
-
 /* The same plus steps a6-a9: the tiny MLPs are evaluated (in the scene's precision mode) and
  *  field   DEVICE float[cap*4]  (sigma, r, g, b) of every sample, in the order of t / subfield
  * is exported before any compositing -- the parity tap for the field (Eq.1, Table 4) sample by sample. */

@@ -81,8 +81,6 @@ def lib():
     L.r360_reserve.argtypes = [vp, C.c_uint64, C.c_double]
     L.r360_set_graph_poses.restype = C.c_int
     L.r360_set_graph_poses.argtypes = [vp, f32p, i32]
-    L.r360_measure_fp32_fma.restype = C.c_int
-    L.r360_measure_fp32_fma.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.r360_set_precision.restype = C.c_int
     L.r360_set_precision.argtypes = [vp, i32]
     L.r360_assign_subfields.restype = C.c_int
@@ -130,9 +128,18 @@ def version():
 
 
 def measure_fp32_fma():
-    """(TFLOP/s, nominal SM MHz) of the FP32 FMA pipes of the current device (r360_measure_fp32_fma)."""
+    """(TFLOP/s, nominal SM MHz) of the FP32 FMA pipes of the current device: bench.py's roofline of the fp32 MLP
+    path.  Lives in libr360_bench.so (csrc/microbench.cu), a measurement helper outside the product ABI."""
+    so = os.path.join(_HERE, "csrc", "libr360_bench.so")
+    if not os.path.exists(so):
+        raise ImportError(f"{so} is missing: run `python -c 'import __graft_entry__ as g; g.build()'`")
+    fn = C.CDLL(so).r360bench_fp32_fma
+    fn.restype = C.c_int
+    fn.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
     tf, mhz = C.c_double(0), C.c_double(0)
-    _check(lib().r360_measure_fp32_fma(C.byref(tf), C.byref(mhz)), "r360_measure_fp32_fma")
+    rc = fn(C.byref(tf), C.byref(mhz))
+    if rc != 0:
+        raise RuntimeError(f"r360bench_fp32_fma failed: cudaError_t {rc}")
     return tf.value, mhz.value
 
 
