@@ -404,7 +404,9 @@ def main():
     precision = args.precision
     if precision == "auto":
         try:
-            scene.set_precision("bf16")          # BASELINE.json's "bf16 tensor-core variant"
+            # BASELINE.json's "bf16 tensor-core variant" is the headline; binary16 operands (mode 2, same kernel and
+            # speed) are the tensor mode for opaque scenes and are reported beside it (f16_same_workload)
+            scene.set_precision("bf16")
             precision = "bf16"
         except r360.R360Error:
             precision = "fp32"
@@ -549,6 +551,16 @@ def main():
             others += [time_config(r360, c, "bf16", peaks, alu_peak, steps=3 if c == 4 else 5) for c in (4, 5)
                        if c != args.config]
             line["other_configs"] = others
+            # the headline dtype is bfloat16 (BASELINE.json's "bf16 tensor-core variant"); the SAME kernel with binary16
+            # operands is the tensor mode for opaque (trained) scenes -- it meets north_star's 2e-3 where a pixel is one
+            # or two samples and bfloat16 does not -- so its line stands beside the headline
+            f16 = next((o for o in others if o["config"] == args.config and o["precision"] == "f16"), None)
+            if f16 is not None and precision == "bf16":
+                line["f16_same_workload"] = {"ms_per_step": f16["ms_per_step"], "rays_per_s": f16["rays_per_s"],
+                                             "fps": f16["fps"], "roofline_frac": f16["roofline"]["frac"],
+                                             "note": "r360_set_precision mode 2: binary16 operands, same tcgen05 kernel; "
+                                                     "the tensor mode for opaque scenes (2e-3 held on them by "
+                                                     "tests/test_gpu_tc.py::test_render_f16_opaque_scenes)"}
         if not args.no_paper_conditions:
             # SURVEY.md 8(f) rows and the paper's own timing condition, device-timed, a few steps each.
             # The paper times its perspective (roaming) view at 720p (Fig. 8 :216 at n = 2048): the same

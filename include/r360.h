@@ -291,9 +291,11 @@ r360_status r360_set_wavefront(r360_scene* scene, int32_t mode);
  *  0 = binary32 on the FP32 ALUs (default; within 1e-4 of the oracle);
  *  1 = tensor cores (tcgen05), operands (weights, positional encoding, activations) rounded to bfloat16,
  *      binary32 accumulation -- BASELINE.json's "bf16 tensor-core variant";
- *  2 = the same kernel with binary16 operands (11 significant bits instead of 8, same speed): the mode for scenes
+ *  2 = the same kernel with binary16 operands (11 significant bits instead of 8, same speed): THE tensor mode for scenes
  *      whose pixels are decided by one or two samples (opaque surfaces), where bfloat16's per-sample colour error
- *      (up to 2.4e-3) is not averaged out; DESIGN.md section 6 has the per-layer error table.
+ *      (up to 2.4e-3, above the 2e-3 bar) is not averaged out; mode 2 stays within 5e-4 there.  Mode 1 is within
+ *      2e-3 only where a pixel averages many samples (all five BASELINE.json scenes).  DESIGN.md section 6 has the
+ *      per-layer error table.
  * R360_ERR_INVALID_ARG: unknown mode; modes 1-2 for a network the tensor kernel does not cover (positional
  * encodings other than L = 10 / 4, or weight buffers that exceed the SM's shared memory: Wd = 32 with more than 6
  * trunk layers, Wd = 64 with more than 3); mode 2 when a weight, a bias or a product of the folded feature and
